@@ -1,0 +1,169 @@
+/*
+ * kara.h — C ABI of libkara: Kara's decoding-time sliding-window KV-cache compression step
+ * (arxiv/paper_2607_01237) on a paged bf16 KV cache, as hand-written CUDA for sm_100a (B200).
+ *
+ * What one kara_compress_window call computes, for every (sequence, layer, KV head) "unit"
+ * of the batch (window-relative 0-based positions; W = |W| window length, U = |U| protected
+ * buffer at the window's end, n = W-U compressible keys, G = n_q_heads / n_kv_heads):
+ *
+ *   a1 score      A_j = sum_{i<W} sum_{g<G} softmax_j( Q[(i,g)] . K[j] / sqrt(d) )      j in [0,n)
+ *                 PAPER.md Eq. 4 (L115): bidirectional (unmasked) attention of ALL window
+ *                 queries against the compressible keys, softmax over keys, colsum over queries.
+ *   a2 top-k      I = the k = keep - alpha best-scoring positions, keep = ceil(r n)
+ *                 PAPER.md Eq. 5 (L117).
+ *   a3 Token2Chunk consecutive members a<b of sorted I are chunk endpoints; eligible iff
+ *                 b-a < gamma; R = (A_a + A_b)(b-a-1); the floor(alpha/(gamma-2)) best eligible
+ *                 chunks add their interiors; the rest of the budget is filled with the best
+ *                 unselected positions                    PAPER.md Eq. 6-8 (L133-138), App. C.3 (L350).
+ *   a4 compaction (K,V)[h .. h+keep) <- (K,V)[h + F[.]], buffer + tail rows follow directly;
+ *                 rows [0,h) are never touched          PAPER.md Eq. 9 (L142), Sec. 4.3 (L150).
+ *   a5 metadata   seq_len <- h+keep+U+t; trailing blocks of the block table are pushed on the
+ *                 device free list and set to -1         PAPER.md Alg. 1 l.11-12 (L336-337), App. C.4 (L354).
+ *
+ * Tie-breaks and the other places where the paper is silent follow DESIGN.md "Readings":
+ * GQA heads are summed (G1); ties -> lower index first (G4); keep = ceil(ratio*n - 1e-9) with
+ * ratio a double (G5); chunk filter before top-P (G7); retained rows keep ascending order (G10).
+ *
+ * Conventions.  Pointers marked [dev] are device memory OWNED BY THE CALLER (e.g. torch
+ * tensors); [host] are host memory.  The library allocates nothing on the device except through
+ * kara_compress_window_host's internal staging buffers.  Calls are asynchronous on `stream`
+ * (a cudaStream_t passed as void*; NULL = legacy default stream) unless marked synchronous.
+ * Every call returns 0 (KARA_OK) or a negative KARA_E* code and never throws or aborts;
+ * kara_last_error() gives a thread-local message for the last failure.  Data-dependent faults
+ * found on the device (a block id outside the pool, a sequence shorter than its window) set bits
+ * in a device status word, the offending unit is skipped, and kara_status() reports the bits.
+ *
+ * Physical layout fixed by kara_init_cache (separate K and V pools, each):
+ *     bf16 pool[n_layers][num_blocks][n_kv_heads][block_size][head_dim]
+ * so one (layer, block, kv_head) tile is block_size*head_dim*2 contiguous bytes (one TMA box
+ * per 64-element column panel).  Logical token p of sequence s lives in block
+ * block_table[s][p / block_size], slot p % block_size, for every layer and head.
+ */
+#ifndef KARA_H
+#define KARA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KARA_OK 0
+#define KARA_EINVAL (-1)       /* bad argument / shape / null pointer */
+#define KARA_EBUDGET (-2)      /* keep - alpha < 1, keep > n, or gamma < 3 */
+#define KARA_EUNSUPPORTED (-3) /* head_dim not in {64,128}, block_size not a power of two in [16,256], n > 2048 */
+#define KARA_ECUDA (-4)        /* a CUDA call or launch failed (message in kara_last_error) */
+#define KARA_ENOMEM (-5)       /* workspace too small */
+
+/* flags of kara_compress_window */
+#define KARA_COMMIT 1u           /* run a5 (seq_lens, block table truncation, free list) after a4.
+                                    Set it only on the call that finishes the LAST layer: blocks must
+                                    not be freed while other layers still hold live rows in them. */
+#define KARA_KEEP_DEBUG 2u       /* keep scores / I / F of every unit in the workspace for kara_gather_debug */
+#define KARA_SCORE_QBUF_ONLY 4u  /* ablation "w/o Bi-Attention": queries = buffer U only */
+#define KARA_SCORE_SIMT 8u       /* force the CUDA-core score kernel (debug cross-check of the tcgen05 path) */
+
+/* `what` of kara_gather_debug */
+#define KARA_DBG_K_LOGICAL 0  /* bf16 [seq_len][d] rows of (layer, seq, kv_head) read through the block table */
+#define KARA_DBG_V_LOGICAL 1
+#define KARA_DBG_SCORES 2     /* fp32 [n]      last call with KARA_KEEP_DEBUG */
+#define KARA_DBG_IDX_TOPK 3   /* int32 [k]     ascending (Eq. 5) */
+#define KARA_DBG_IDX_FINAL 4  /* int32 [keep]  ascending (Eq. 8 + C.3) */
+#define KARA_DBG_BLOCK_TABLE_ROW 5 /* int32 [max_blocks] */
+#define KARA_DBG_FREE_LIST 6  /* int32 [free_count] */
+
+/* bits of the device status word */
+#define KARA_ST_BAD_BLOCK 1   /* a block-table entry touched by the window is outside [0, num_blocks) */
+#define KARA_ST_SHORT_SEQ 2   /* win_start < 0 or win_start + W > seq_len */
+#define KARA_ST_TABLE_OVERFLOW 4 /* ceil(seq_len / block_size) > max_blocks */
+
+typedef struct kara_cache kara_cache;
+
+/* Fix the geometry of the paged cache.  Returns a handle (host object, no device allocation) or
+ * NULL (kara_last_error says why: KARA_EUNSUPPORTED shapes).  PAPER.md:L82 (PagedAttention blocks). */
+kara_cache* kara_init_cache(int block_size, int n_layers, int n_kv_heads, int head_dim);
+
+/* Frees the handle and any staging buffers kara_compress_window_host allocated.  Synchronous. */
+void kara_destroy(kara_cache* c);
+
+/* Bytes of one pool (K or V) with num_blocks blocks, and of one block across all layers' slices. */
+int64_t kara_pool_bytes(const kara_cache* c, int64_t num_blocks);
+int64_t kara_block_bytes(const kara_cache* c);
+
+/* Attach caller-owned device memory: the two pools (layout above, 256-byte aligned) and the
+ * free list: free_list [dev int32 num_blocks] is a stack whose first *free_count entries are the
+ * free block ids; a5 appends to it.  Must be called before kara_compress_window.  Synchronous
+ * (builds the TMA descriptor of the K pool). */
+int kara_attach_pool(kara_cache* c, void* k_pool /*dev*/, void* v_pool /*dev*/, int64_t num_blocks,
+                     int32_t* free_list /*dev*/, int32_t* free_count /*dev [1]*/);
+
+/* keep = ceil(ratio * n) evaluated as (int)ceil(ratio*n - 1e-9) (reading G5); <0 on bad input. */
+int kara_budget(int n, double ratio);
+
+/* Bytes of device scratch kara_compress_window needs for this geometry. */
+size_t kara_workspace_bytes(const kara_cache* c, int n_layers_in_call, int n_seqs, int n_q_heads,
+                            int W, int U, double ratio, int alpha);
+
+/* The batched compression step: a1-a4 for layers [layer_begin, layer_end) x n_seqs sequences x
+ * all KV heads, and a5 if flags & KARA_COMMIT.
+ *   block_table [dev int32 n_seqs x max_blocks] in/out   -1 padded; freed entries become -1
+ *   seq_lens    [dev int32 n_seqs]              in/out   tokens currently stored per sequence
+ *   win_start   [dev int32 n_seqs] or NULL      in       h: first token of the window; NULL => seq_len - W.
+ *                                                        t = seq_len - h - W tail tokens (App. C.4's partial
+ *                                                        last block) are carried over behind the buffer.
+ *   window_q    [dev bf16 (layer_end-layer_begin) x n_seqs x W x n_q_heads x head_dim]  in
+ *                                                        query states of the window tokens,
+ *                                                        16-byte aligned
+ *   ratio, alpha, gamma                                  r, chunk budget, max chunk length (Eq. 5-7)
+ *   workspace   [dev] >= kara_workspace_bytes(...), 256-byte aligned; contents are scratch
+ * All sequences share W, U, ratio, alpha, gamma.  After the call the last U tokens of
+ * the old window are the first U uncompressed tokens behind the retained ones. */
+int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_seqs,
+                         int32_t* block_table /*dev*/, int max_blocks, int32_t* seq_lens /*dev*/,
+                         const int32_t* win_start /*dev or NULL*/, const void* window_q /*dev*/,
+                         int n_q_heads, int W, int U, double ratio, int alpha, int gamma,
+                         unsigned flags, void* workspace /*dev*/, size_t workspace_bytes,
+                         void* stream);
+
+/* Same step with HOST buffers for everything but the resident pools: copies window_q,
+ * block_table, seq_lens, win_start host->device into library-owned staging buffers, runs
+ * kara_compress_window on `stream`, copies block_table and seq_lens back and reports the new
+ * free count.  Synchronous on return.  Host buffers should be pinned for full copy bandwidth. */
+int kara_compress_window_host(kara_cache* c, int layer_begin, int layer_end, int n_seqs,
+                              int32_t* block_table /*host in/out*/, int max_blocks,
+                              int32_t* seq_lens /*host in/out*/, const int32_t* win_start /*host or NULL*/,
+                              const void* window_q /*host*/, int n_q_heads, int W, int U, double ratio,
+                              int alpha, int gamma, unsigned flags, int32_t* free_count_out /*host [1] or NULL*/,
+                              void* stream);
+
+/* Synchronous read-back for tests: writes up to out_capacity_bytes to `out` [host] and the
+ * number of ELEMENTS written to *out_count.  SCORES / IDX_* refer to the unit (layer, seq, kv_head)
+ * of the last kara_compress_window call made with KARA_KEEP_DEBUG (layer is absolute). */
+int kara_gather_debug(kara_cache* c, int what, int layer, int seq, int kv_head,
+                      const int32_t* block_table /*dev*/, const int32_t* seq_lens /*dev*/,
+                      int max_blocks, void* out /*host*/, int64_t out_capacity_bytes,
+                      int64_t* out_count /*host*/);
+
+/* Synchronous: reads and clears the device status word of the last call (0 = no fault). */
+int kara_status(kara_cache* c, int32_t* status_out /*host*/);
+
+/* Number of kernel launches the last kara_compress_window call made (for bench.py's gpu_launches). */
+int kara_last_launch_count(const kara_cache* c);
+
+/* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA. */
+int kara_last_score_path(const kara_cache* c);
+
+/* Device time of the score kernel (a1) alone: when enabled, every kara_compress_window call
+ * brackets its score launch with CUDA events on `stream`; kara_score_kernel_ms() synchronises on
+ * the last pair and returns its milliseconds (<0 if none).  Used for bench.py's roofline object. */
+int kara_enable_score_timing(kara_cache* c, int enable);
+float kara_score_kernel_ms(kara_cache* c);
+
+/* Thread-local message for the last failing call on this thread ("" if none). */
+const char* kara_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KARA_H */

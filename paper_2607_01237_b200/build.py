@@ -1,0 +1,56 @@
+"""Build libkara.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+    python -m paper_2607_01237_b200.build [--force] [--verbose]
+
+One nvcc -c per csrc/*.cu (skipped when the object is newer than every source/header), then a
+shared link with the static CUDA runtime, so the library loads on a machine without a driver
+(symbols resolve; calls fail with a CUDA error).  The driver API entry point the TMA descriptors
+need is fetched at run time through cudaGetDriverEntryPoint, so there is no link against libcuda.
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+from pathlib import Path
+
+HERE = Path(__file__).resolve().parent
+CSRC = HERE / "csrc"
+OBJ = HERE / "build"
+SO = HERE / "libkara.so"
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+         "-Xcompiler", "-fPIC,-Wall,-Wextra", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    OBJ.mkdir(exist_ok=True)
+    hdrs = list(CSRC.glob("*.h")) + [HERE.parent / "include" / "kara.h"]
+    newest_hdr = max(p.stat().st_mtime for p in hdrs)
+    objs, rebuilt = [], False
+    for cu in sorted(CSRC.glob("*.cu")):
+        o = OBJ / (cu.stem + ".o")
+        objs.append(o)
+        if force or not o.exists() or o.stat().st_mtime < max(cu.stat().st_mtime, newest_hdr):
+            cmd = [NVCC, *FLAGS, "-c", str(cu), "-o", str(o)]
+            r = subprocess.run(cmd, capture_output=True, text=True)
+            if verbose or r.returncode:
+                sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+            if r.returncode:
+                raise RuntimeError(f"nvcc failed on {cu.name}")
+            (OBJ / (cu.stem + ".ptxas.txt")).write_text(r.stderr)
+            rebuilt = True
+    if rebuilt or not SO.exists():
+        tmp = SO.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static",
+               *map(str, objs), "-o", str(tmp)]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode:
+            sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+            raise RuntimeError("link failed")
+        os.replace(tmp, SO)
+    return SO
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

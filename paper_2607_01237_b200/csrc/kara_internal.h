@@ -1,0 +1,92 @@
+// kara_internal.h — shared declarations of libkara's translation units (not part of the ABI).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/kara.h"
+
+namespace kara {
+
+// Geometry of the paged pool (include/kara.h "Physical layout"), strides in bf16 elements.
+struct Geom {
+  int bs, bs_log2, n_layers, n_kv_heads, d;
+  long long num_blocks;
+  long long sL, sB, sH;  // layer, block, head strides; slot stride = d
+};
+
+// Parameters of one compress_window call, passed by value to every kernel.
+struct Call {
+  Geom g;
+  const __nv_bfloat16* k_pool;
+  const __nv_bfloat16* v_pool;  // written by the compaction kernel through a non-const alias
+  int layer_begin, n_layers, n_seqs, max_blocks;
+  int n_q_heads, G, W, U, n, keep, k, P, alpha, gamma;
+  int q_row_begin;  // first window token used as a query (0, or W-U with KARA_SCORE_QBUF_ONLY)
+  int32_t* block_table;
+  int32_t* seq_lens;
+  const int32_t* win_start;
+  const __nv_bfloat16* window_q;
+  // workspace pieces
+  int32_t* status;   // [8]
+  float* partial;    // [units][parts][n_pad]
+  float* scores;     // [units][n_pad]
+  int32_t* idx_topk; // [units][k_pad]
+  int32_t* idx_final;// [units][keep_pad]
+  int parts, n_pad, k_pad, keep_pad;
+  int keep_debug;
+  int32_t* free_list;
+  int32_t* free_count;
+};
+
+struct WsLayout {
+  size_t status_off, partial_off, scores_off, topk_off, final_off, total;
+  int parts, n_pad, k_pad, keep_pad;
+};
+
+constexpr int kMaxParts = 16;   // partial column sums per unit, reduced in fixed order by select
+constexpr int kMaxN = 2048;     // largest compressible region (cfg 5: 1984)
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// unit index -> (layer-in-call, sequence, kv head)
+__host__ __device__ inline void unit_decode(int unit, int n_seqs, int n_kv_heads, int& li, int& s, int& hk) {
+  hk = unit % n_kv_heads;
+  s = (unit / n_kv_heads) % n_seqs;
+  li = unit / (n_kv_heads * n_seqs);
+}
+
+// Window geometry of sequence s, validated on the device.  Returns false (and sets status bits)
+// if the unit must be skipped.
+__device__ inline bool window_of(const Call& c, int s, int& h, int& t, int& len) {
+  len = c.seq_lens[s];
+  h = c.win_start ? c.win_start[s] : len - c.W;
+  t = len - h - c.W;
+  int bad = 0;
+  if (h < 0 || t < 0) bad |= KARA_ST_SHORT_SEQ;
+  if (((len + c.g.bs - 1) >> c.g.bs_log2) > c.max_blocks) bad |= KARA_ST_TABLE_OVERFLOW;
+  if (bad) { atomicOr(c.status, bad); return false; }
+  return true;
+}
+
+// Element offset of logical token `pos` of sequence s, head hk, in layer `layer` (absolute).
+// Returns -1 (and sets the status bit) if the block id is outside the pool.
+__device__ inline long long row_offset(const Call& c, int layer, int s, int hk, int pos) {
+  const int blk = c.block_table[(long long)s * c.max_blocks + (pos >> c.g.bs_log2)];
+  if (blk < 0 || blk >= c.g.num_blocks) { atomicOr(c.status, KARA_ST_BAD_BLOCK); return -1; }
+  return (long long)layer * c.g.sL + (long long)blk * c.g.sB + (long long)hk * c.g.sH +
+         (long long)(pos & (c.g.bs - 1)) * c.g.d;
+}
+
+// kernel launchers (each returns the cudaError_t of its launch)
+cudaError_t launch_score_simt(const Call& c, cudaStream_t st);
+cudaError_t launch_select_compact(const Call& c, cudaStream_t st);
+cudaError_t launch_metadata(const Call& c, cudaStream_t st);
+cudaError_t launch_gather_rows(const Geom& g, const __nv_bfloat16* pool, int layer, int kv_head,
+                               const int32_t* bt_row, int length, __nv_bfloat16* out, int32_t* status,
+                               cudaStream_t st);
+size_t select_compact_smem_bytes(const Call& c, int moved_rows_hint);
+
+}  // namespace kara

@@ -1,0 +1,289 @@
+// select_compact.cu — a2 + a3 + a4 for one (sequence, layer, KV head) unit per CTA.
+//
+//   a2  Eq. 5   I = top-(keep-alpha) of A under (A desc, index asc)
+//   a3  Eq. 6-8 (L133-138) + App. C.3 (L350): eligible chunks (b-a < gamma, interior >= 1),
+//       R = fl32(fl32(A_a + A_b) * gap), top-P under (R desc, ordinal asc), interiors added,
+//       budget filled with the best unselected positions under (A desc, index asc)
+//   a4  Eq. 9 (L142): rows h+F[c] -> h+c for K and V, buffer + tail rows behind them, in place
+//
+// Every TopK is the same block-wide primitive: an 8-bit-digit radix select over the
+// order-preserving integer image of the fp32 key (4 passes, 256-bin shared-memory histogram,
+// bins scanned by one warp with shuffles), then the tie class (key == threshold) is resolved in
+// index order with a ballot-free segmented count + block scan.  All decisions are integer
+// compares on fp32 bit patterns, so the result is a pure function of the scores.
+//
+// In-place compaction is hazard-free with one CTA per (unit, tensor): destination c <= source
+// F[c] and both are increasing, so staging rows [c0,c1) in shared memory, barrier, then writing
+// them never overwrites a row a later chunk still has to read.
+#include "kara_internal.h"
+
+namespace kara {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+
+struct Scratch {
+  int hist[256];
+  int warp_tot[kWarps];
+  unsigned prefix, mask;
+  int remaining;
+  int bcast;
+};
+
+__device__ __forceinline__ unsigned key_of(float x) {
+  const unsigned b = __float_as_uint(x);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+// exclusive scan of one int per thread over the block; returns the exclusive prefix, total in *total
+__device__ __forceinline__ int block_excl_scan(int v, Scratch* sc, int* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += y;
+  }
+  __syncthreads();  // protect warp_tot from a previous use
+  if (lane == 31) sc->warp_tot[warp] = inc;
+  __syncthreads();
+  int base = 0, tot = 0;
+#pragma unroll
+  for (int w = 0; w < kWarps; ++w) {
+    const int x = sc->warp_tot[w];
+    if (w < warp) base += x;
+    tot += x;
+  }
+  *total = tot;
+  return base + inc - v;
+}
+
+// Marks sel[i] = 1 for the m best of the N candidates with valid(i), under (key desc, i asc).
+// Requires 0 <= m <= #valid.  key/sel live in shared memory.  Block-wide; ends synchronised.
+template <typename Valid>
+__device__ void block_top_m(const unsigned* key, int N, int m, Valid valid, unsigned char* sel, Scratch* sc) {
+  if (m <= 0) { __syncthreads(); return; }
+  const int tid = threadIdx.x;
+  if (tid == 0) { sc->prefix = 0u; sc->mask = 0u; sc->remaining = m; }
+  for (int pass = 3; pass >= 0; --pass) {
+    const int shift = pass * 8;
+    sc->hist[tid] = 0;   // kThreads == 256 bins
+    __syncthreads();
+    const unsigned prefix = sc->prefix, mask = sc->mask;
+    for (int i = tid; i < N; i += kThreads)
+      if (valid(i) && (key[i] & mask) == prefix) atomicAdd(&sc->hist[(key[i] >> shift) & 255u], 1);
+    __syncthreads();
+    if (tid < 32) {
+      // lane l owns bins 255-8l .. 248-8l (descending); find the bin where the running count
+      // from the top first reaches `remaining`
+      const int remaining = sc->remaining;
+      int loc[8], sum = 0;
+#pragma unroll
+      for (int b = 0; b < 8; ++b) { loc[b] = sc->hist[255 - 8 * tid - b]; sum += loc[b]; }
+      int inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, inc, o);
+        if (tid >= o) inc += y;
+      }
+      int above = inc - sum;  // candidates in strictly higher bins than this lane's
+      if (above < remaining && inc >= remaining) {
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+          if (above + loc[b] >= remaining) {
+            sc->prefix = prefix | ((unsigned)(255 - 8 * tid - b) << shift);
+            sc->mask = mask | (255u << shift);
+            sc->remaining = remaining - above;
+            break;
+          }
+          above += loc[b];
+        }
+      }
+    }
+    __syncthreads();
+  }
+  // threshold key T = sc->prefix; everything above T is selected, plus the first `r` (index
+  // order) of the tie class key == T
+  const unsigned T = sc->prefix;
+  const int r = sc->remaining;
+  const int seg = (N + kThreads - 1) / kThreads;
+  const int i0 = min(N, tid * seg), i1 = min(N, i0 + seg);
+  int eq = 0;
+  for (int i = i0; i < i1; ++i) eq += (valid(i) && key[i] == T) ? 1 : 0;
+  int total;
+  int rank = block_excl_scan(eq, sc, &total);
+  for (int i = i0; i < i1; ++i) {
+    if (!valid(i)) continue;
+    const unsigned ki = key[i];
+    if (ki > T) sel[i] = 1;
+    else if (ki == T) { if (rank < r) sel[i] = 1; ++rank; }
+  }
+  __syncthreads();
+}
+
+// ascending list of the set positions of flag[0..N) -> out[]; returns the count.  Block-wide.
+__device__ int block_compact(const unsigned char* flag, int N, int* out, Scratch* sc) {
+  const int tid = threadIdx.x;
+  const int seg = (N + kThreads - 1) / kThreads;
+  const int i0 = min(N, tid * seg), i1 = min(N, i0 + seg);
+  int cnt = 0;
+  for (int i = i0; i < i1; ++i) cnt += flag[i] ? 1 : 0;
+  int total;
+  int pos = block_excl_scan(cnt, sc, &total);
+  for (int i = i0; i < i1; ++i) if (flag[i]) out[pos++] = i;
+  __syncthreads();
+  return total;
+}
+
+// plain (coherent) streaming load: the pool is written by this kernel, so no .nc
+__device__ __forceinline__ uint4 ld_stream16(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_na16(void* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+               :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+__global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, int stage_rows) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = c.n, n_pad = c.n_pad, k = c.k, keep = c.keep, d = c.g.d;
+  // carve
+  uint4* s_stage = reinterpret_cast<uint4*>(smem_raw);                         // [stage_rows][d*2/16]
+  const int vpr = d / 8;                                                       // 16-byte vectors per row
+  float* s_A = reinterpret_cast<float*>(s_stage + (size_t)stage_rows * vpr);   // [n_pad]
+  unsigned* s_key = reinterpret_cast<unsigned*>(s_A + n_pad);                  // [n_pad]
+  int* s_I = reinterpret_cast<int*>(s_key + n_pad);                            // [k_pad]
+  int* s_F = s_I + c.k_pad;                                                    // [keep_pad]
+  unsigned* s_rkey = reinterpret_cast<unsigned*>(s_F + c.keep_pad);            // [k_pad] chunk keys
+  Scratch* sc = reinterpret_cast<Scratch*>(s_rkey + c.k_pad);
+  unsigned char* s_sel = reinterpret_cast<unsigned char*>(sc + 1);             // [n_pad] retained flag
+  unsigned char* s_csel = s_sel + n_pad;                                       // [k_pad] chunk flags
+  unsigned char* s_celig = s_csel + c.k_pad;                                   // [k_pad]
+
+  const int unit = blockIdx.x, tid = threadIdx.x;
+  int li, s, hk;
+  unit_decode(unit, c.n_seqs, c.g.n_kv_heads, li, s, hk);
+  const int layer = c.layer_begin + li;
+
+  int h, t, len;
+  if (!window_of(c, s, h, t, len)) return;   // uniform per CTA
+
+  // ---- scores: sum the score kernel's partial column sums in part order -------------------
+  const float* part = c.partial + (long long)unit * c.parts * n_pad;
+  for (int j = tid; j < n_pad; j += kThreads) {
+    float a = 0.f;
+    if (j < n) for (int p = 0; p < c.parts; ++p) a += part[(long long)p * n_pad + j];
+    s_A[j] = a;
+    s_key[j] = key_of(a);
+    s_sel[j] = 0;
+    if (c.keep_debug && j < n) c.scores[(long long)unit * n_pad + j] = a;
+  }
+  for (int x = tid; x < c.k_pad; x += kThreads) { s_csel[x] = 0; s_celig[x] = 0; s_rkey[x] = 0u; }
+  __syncthreads();
+
+  // ---- a2: I = top-k (Eq. 5) ----------------------------------------------------------------
+  block_top_m(s_key, n, k, [](int) { return true; }, s_sel, sc);
+  block_compact(s_sel, n, s_I, sc);
+  if (c.keep_debug) for (int x = tid; x < k; x += kThreads) c.idx_topk[(long long)unit * c.k_pad + x] = s_I[x];
+
+  // ---- a3: Token2Chunk (Eq. 6-8) --------------------------------------------------------------
+  int n_elig_local = 0;
+  for (int x = tid; x < k - 1; x += kThreads) {
+    const int a = s_I[x], b = s_I[x + 1];
+    const int gap = b - a - 1;
+    if (b - a < c.gamma && gap >= 1) {
+      const float r = __fmul_rn(__fadd_rn(s_A[a], s_A[b]), (float)gap);   // Eq. 6, no contraction
+      s_rkey[x] = key_of(r);
+      s_celig[x] = 1;
+      ++n_elig_local;
+    }
+  }
+  int n_elig;
+  block_excl_scan(n_elig_local, sc, &n_elig);
+  __syncthreads();
+  const int n_pick = min(c.P, n_elig);
+  {
+    const unsigned char* elig = s_celig;
+    block_top_m(s_rkey, k - 1, n_pick, [elig](int x) { return elig[x] != 0; }, s_csel, sc);
+  }
+  int added_local = 0;
+  for (int x = tid; x < k - 1; x += kThreads)
+    if (s_csel[x]) {
+      for (int j = s_I[x] + 1; j < s_I[x + 1]; ++j) { s_sel[j] = 1; ++added_local; }   // Eq. 8
+    }
+  int added;
+  block_excl_scan(added_local, sc, &added);
+  __syncthreads();
+
+  // ---- App. C.3 fill --------------------------------------------------------------------------
+  {
+    // Candidates are the positions unselected before the fill.  The histogram passes need a
+    // stable candidate set, so the fill selects into its own flag array (the staging area is
+    // free until a4) and the flags are merged afterwards.
+    const unsigned char* selc = s_sel;
+    unsigned char* fillflag = reinterpret_cast<unsigned char*>(s_stage);
+    for (int j = tid; j < n; j += kThreads) fillflag[j] = 0;
+    __syncthreads();
+    block_top_m(s_key, n, keep - k - added, [selc](int j) { return selc[j] == 0; }, fillflag, sc);
+    for (int j = tid; j < n; j += kThreads) if (fillflag[j]) s_sel[j] = 1;
+    __syncthreads();
+  }
+  block_compact(s_sel, n, s_F, sc);   // F: ascending (reading G10), |F| = keep
+  if (c.keep_debug) for (int x = tid; x < keep; x += kThreads) c.idx_final[(long long)unit * c.keep_pad + x] = s_F[x];
+
+  // ---- a4: compaction of K then V (Eq. 9), staged through shared memory ------------------------
+  const int moved = keep + c.U + t;
+  for (int which = 0; which < 2; ++which) {
+    __nv_bfloat16* pool = const_cast<__nv_bfloat16*>(which == 0 ? c.k_pool : c.v_pool);
+    for (int c0 = 0; c0 < moved; c0 += stage_rows) {
+      const int rows = min(stage_rows, moved - c0);
+      for (int x = tid; x < rows * vpr; x += kThreads) {
+        const int row = c0 + x / vpr, v = x % vpr;
+        const int src = row < keep ? h + s_F[row] : h + n + (row - keep);
+        const long long off = row_offset(c, layer, s, hk, src);
+        s_stage[x] = off >= 0 ? ld_stream16(pool + off + v * 8) : make_uint4(0, 0, 0, 0);
+      }
+      __syncthreads();
+      for (int x = tid; x < rows * vpr; x += kThreads) {
+        const int row = c0 + x / vpr, v = x % vpr;
+        const long long off = row_offset(c, layer, s, hk, h + row);
+        if (off >= 0) st_na16(pool + off + v * 8, s_stage[x]);
+      }
+      __syncthreads();
+    }
+  }
+}
+
+size_t smem_bytes(const Call& c, int stage_rows) {
+  size_t b = (size_t)stage_rows * c.g.d * 2;
+  b += sizeof(float) * c.n_pad + sizeof(unsigned) * c.n_pad;
+  b += sizeof(int) * (c.k_pad + c.keep_pad) + sizeof(unsigned) * c.k_pad;
+  b += sizeof(Scratch);
+  b += (size_t)c.n_pad + 2 * (size_t)c.k_pad;
+  return (b + 15) / 16 * 16;
+}
+
+}  // namespace
+
+cudaError_t launch_select_compact(const Call& c, cudaStream_t st) {
+  const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;
+  // stage the whole moved range when it fits (keep + U + a little tail), else chunk
+  const int rowB = c.g.d * 2;
+  int stage_rows = c.keep + c.U + 2 * c.g.bs;
+  const int cap_rows = (160 * 1024) / rowB;
+  if (stage_rows > cap_rows) stage_rows = cap_rows;
+  // the staging area doubles as the fill-flag array (n bytes)
+  if (stage_rows * rowB < c.n_pad) stage_rows = (c.n_pad + rowB - 1) / rowB;
+  const size_t smem = smem_bytes(c, stage_rows);
+  cudaError_t e = cudaFuncSetAttribute(select_compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  select_compact_kernel<<<units, kThreads, smem, st>>>(c, stage_rows);
+  return cudaGetLastError();
+}
+
+}  // namespace kara

@@ -1,0 +1,84 @@
+"""The C-ABI library builds, loads and exports every symbol include/kara.h declares — CPU only
+(no compute calls: only the host-side entry points that touch no CUDA API are exercised)."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def kara():
+    from paper_2607_01237_b200 import build, kara as k
+    build.build()
+    k.lib()
+    return k
+
+
+def _declared_symbols():
+    text = (ROOT / "include" / "kara.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(kara_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported_and_bound(kara):
+    declared = _declared_symbols()
+    assert len(declared) >= 14 and "kara_init_cache" in declared and "kara_compress_window" in declared \
+        and "kara_gather_debug" in declared
+    L = kara.lib()
+    for name in declared:
+        assert hasattr(L, name), f"libkara.so does not export {name}"
+        assert name in kara.SYMBOLS, f"binding has no signature for {name}"
+    assert sorted(kara.SYMBOLS) == declared
+
+
+def test_no_torch_or_python_types_in_the_abi():
+    text = (ROOT / "include" / "kara.h").read_text()
+    assert 'extern "C"' in text
+    code = re.sub(r"/\*.*?\*/", "", text, flags=re.S)      # declarations only, comments stripped
+    assert "torch" not in code.lower() and "at::" not in code and "PyObject" not in code and "std::" not in code
+
+
+def test_library_does_not_link_the_oracle(kara):
+    import subprocess
+    so = ROOT / "paper_2607_01237_b200" / "libkara.so"
+    syms = subprocess.run(["nm", "-D", str(so)], capture_output=True, text=True).stdout
+    assert "kara_oracle" not in syms
+
+
+def test_budget_matches_exact_rational(kara):
+    import math
+    from fractions import Fraction
+    for pct in range(5, 101, 5):
+        for n in (56, 192, 224, 352, 480, 736, 992, 1984):
+            assert kara.kara_budget(n, pct / 100) == math.ceil(Fraction(pct, 100) * n)
+    assert kara.kara_budget(0, 0.2) < 0 and kara.kara_budget(10, 0.0) < 0 and kara.kara_budget(10, 1.5) < 0
+
+
+def test_init_cache_geometry_and_errors(kara):
+    L = kara.lib()
+    h = L.kara_init_cache(16, 40, 8, 128)
+    assert h
+    assert L.kara_block_bytes(h) == 40 * 8 * 16 * 128 * 2
+    assert L.kara_pool_bytes(h, 1000) == 40 * 1000 * 8 * 16 * 128 * 2
+    ws = L.kara_workspace_bytes(h, 40, 1, 40, 512, 32, 0.2, 32)
+    assert ws > 320 * 480 * 4 and ws % 256 == 0
+    assert L.kara_last_launch_count(h) == 0 and L.kara_last_score_path(h) == 0
+    # compress before attach is an argument error, not a crash
+    rc = L.kara_compress_window(h, 0, 1, 1, 1, 1, 1, None, 1, 40, 512, 32, 0.2, 32, 8, 0, 1, 0, None)
+    assert rc == kara.KARA_EINVAL and b"attach" in L.kara_last_error()
+    rc = L.kara_compress_window(h, 0, 1, 1, 1, 1, 1, None, 1, 40, 512, 32, 0.2, 96, 8, 0, 1, 0, None)
+    assert rc == kara.KARA_EBUDGET
+    L.kara_destroy(h)
+    for bad in [(15, 1, 1, 128), (16, 1, 1, 96), (512, 1, 1, 128), (16, 0, 1, 128)]:
+        assert not L.kara_init_cache(*bad)
+        assert L.kara_last_error() != b""
+
+
+def test_binding_fails_loudly_without_the_library(kara, monkeypatch, tmp_path):
+    monkeypatch.setattr(kara, "_LIB", None)
+    monkeypatch.setattr(kara, "_SO", tmp_path / "missing.so")
+    with pytest.raises(kara.KaraError):
+        kara.lib()

@@ -1,0 +1,231 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle — needs a B200.
+
+Stages S1/S2/S3 are defined in oracle/check.py and DESIGN.md §Parity.  Tolerance (north_star):
+scores within 1e-3 relative (+1e-6 x mean-score floor, reading G15) with fp32 accumulation; index
+sets identical except at oracle near-ties < 1e-3; given the indices, K/V bytes, block tables,
+seq_lens and the free list bit-exact.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_01237_b200 import inputs as kin
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_01237_b200 import kara
+    import gpu_util
+    kara.lib()
+    return kara, gpu_util
+
+
+@pytest.fixture(scope="module")
+def chk(oracle):
+    from oracle import check
+    return check
+
+
+def _parity(gpu, chk, wl, flags_extra=0, overrides=None, lb=None, le=None, use_win_start=True, check_s1=True):
+    kara, gu = gpu
+    sh = wl.shape
+    p = dict(W=sh.W, U=sh.U, ratio=sh.ratio, alpha=sh.alpha, gamma=sh.gamma)
+    p.update(overrides or {})
+    H0 = chk.host_image(wl)
+    L = H0["k"].shape[0]
+    lb = 0 if lb is None else lb
+    le = L if le is None else le
+    flags = kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG | flags_extra
+    out, cache, _ = gu.gpu_compress(wl, lb, le, flags=flags, use_win_start=use_win_start, overrides=overrides)
+    assert out["status"] == 0
+    stats = chk.compare(H0, out, sh.n_q_heads, p["W"], p["U"], p["ratio"], p["alpha"], p["gamma"], lb, le,
+                        commit=True, check_s1=check_s1)
+    stats["score_path"] = cache.last_score_path()
+    return stats, out, H0
+
+
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", [1, 2, 3, 7, 11, 23, 42, 64])
+def test_cfg1_tiny(gpu, chk, seed):
+    """BASELINE.json configs[0]: 1 seq, 1 layer, GQA 4/1, d=64, bs=16, h=256, W=64, r=20 %."""
+    stats, out, _ = _parity(gpu, chk, kin.generate(kin.CFG1, seed=seed))
+    assert stats["keep"] == 12 and stats["s3_hard_mismatch"] == 0
+    # the planted keys are retained
+    wl = kin.generate(kin.CFG1, seed=seed)
+    planted = set(np.flatnonzero(wl.salient[0].numpy()).tolist())
+    assert planted <= set(out["idx_final"][0, 0, 0].tolist())
+
+
+@pytest.mark.parametrize("simt", [False, True])
+def test_cfg2_shape_two_layers(gpu, chk, simt):
+    """configs[1] shape (40/8 heads, d=128, W=512, U=32, h=4096, alpha=32, gamma=8), 2 of 40 layers:
+    spans several row tiles, 31 key blocks and a ragged window start."""
+    kara, _ = gpu
+    wl = kin.generate(kin.scaled(kin.CFG2, n_layers=2, hist_lo=4099, hist_hi=4099), seed=2)
+    stats, out, _ = _parity(gpu, chk, wl, flags_extra=kara.KARA_SCORE_SIMT if simt else 0)
+    assert stats["keep"] == 96
+    assert stats["score_path"] == (1 if simt else stats["score_path"])
+    assert out["sl"][0] == 4099 + 96 + 32
+    assert int(out["fc"][0]) - int(wl.free_count[0]) == math.ceil((4099 + 512) / 16) - math.ceil((4099 + 128) / 16)
+
+
+def test_batch_ragged_histories_and_tails(gpu, chk):
+    """configs[2]-like batch: independent histories (not block aligned), permuted block tables over
+    a shared pool, tails t in 0..15 (App. C.4's partial last block)."""
+    wl = kin.generate(kin.scaled(kin.CFG3, n_seqs=6, n_layers=2, hist_lo=100, hist_hi=900, tail_lo=0, tail_hi=15),
+                      seed=3)
+    stats, out, H0 = _parity(gpu, chk, wl)
+    assert stats["units"] == 2 * 6 * 8
+    # blocks not touched by any window are byte-identical (history never recompressed)
+    bs = wl.shape.block_size
+    touched = np.zeros(wl.num_blocks, bool)
+    for s in range(6):
+        h, ln = int(H0["ws"][s]), int(H0["sl"][s])
+        touched[H0["bt"][s, h // bs: math.ceil(ln / bs)]] = True
+    np.testing.assert_array_equal(out["k"][:, ~touched], H0["k"][:, ~touched])
+    np.testing.assert_array_equal(out["v"][:, ~touched], H0["v"][:, ~touched])
+    live = np.concatenate([out["bt"][s][out["bt"][s] >= 0] for s in range(6)])
+    allb = np.concatenate([live, out["fl"][: int(out["fc"][0])]])
+    assert sorted(allb.tolist()) == list(range(wl.num_blocks))
+
+
+@pytest.mark.parametrize("ratio,alpha,gamma", [(0.1, 32, 8), (0.3, 32, 8), (0.2, 0, 8), (0.2, 16, 8),
+                                               (0.4, 32, 4), (1.0, 0, 3), (0.5, 112, 16)])
+def test_retention_and_chunk_parameter_sweep(gpu, chk, ratio, alpha, gamma):
+    """r swept as in configs[3]; alpha=0 is 'w/o Token2Chunk'; r=1 is a no-op."""
+    wl = kin.generate(kin.scaled(kin.CFG3, n_seqs=3, n_layers=1, hist_lo=37, hist_hi=300, ratio=ratio,
+                                 alpha=alpha, gamma=gamma), seed=5)
+    stats, out, H0 = _parity(gpu, chk, wl)
+    if ratio == 1.0:
+        np.testing.assert_array_equal(out["k"], H0["k"])
+        np.testing.assert_array_equal(out["bt"], H0["bt"])
+
+
+def test_w1024_window(gpu, chk):
+    """configs[3] window (W=1024, U=32, n=992, keep=199): keys beyond one CTA's TMEM."""
+    wl = kin.generate(kin.scaled(kin.CFG4, n_seqs=2, n_layers=1, hist_lo=50, hist_hi=400, pool_slack=1.1), seed=4)
+    stats, _, _ = _parity(gpu, chk, wl)
+    assert stats["keep"] == 199
+
+
+def test_w2048_student_t_stress(gpu, chk):
+    """configs[4] shape: 64/8 heads, W=2048, U=64 (n=1984, keep=397), Student-t(3) keys: |logit|~80."""
+    wl = kin.generate(kin.scaled(kin.CFG5, n_seqs=1, n_layers=1, hist_lo=77, hist_hi=77), seed=5)
+    stats, _, _ = _parity(gpu, chk, wl)
+    assert stats["keep"] == 397
+
+
+def test_layer_range_call_then_commit(gpu, chk):
+    """Layers compressed in two calls; only the last one commits metadata (include/kara.h)."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_seqs=2, n_layers=3, n_q_heads=4, n_kv_heads=2, hist_lo=30, hist_hi=80),
+                      seed=8)
+    sh = wl.shape
+    H0 = chk.host_image(wl)
+    D = gu.to_cuda(wl)
+    cache = kara.KaraCache(sh.block_size, 3, sh.n_kv_heads, sh.head_dim)
+    cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+    args = (sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma)
+    cache.compress_window(0, 2, D["bt"], D["sl"], D["ws"], D["q"][0:2].contiguous(), *args, flags=kara.KARA_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    a = gu.readback(cache, D, 0, 2, sh.n_seqs, sh.n_kv_heads, kara.KARA_KEEP_DEBUG)
+    np.testing.assert_array_equal(a["bt"], H0["bt"])      # nothing committed yet
+    np.testing.assert_array_equal(a["sl"], H0["sl"])
+    cache.compress_window(2, 3, D["bt"], D["sl"], D["ws"], D["q"][2:3].contiguous(), *args,
+                          flags=kara.KARA_KEEP_DEBUG | kara.KARA_COMMIT)
+    torch.cuda.synchronize()
+    b = gu.readback(cache, D, 2, 3, sh.n_seqs, sh.n_kv_heads, kara.KARA_KEEP_DEBUG)
+    merged = dict(b)
+    for key in ("scores", "idx_topk", "idx_final"):
+        merged[key] = np.concatenate([a[key], b[key]], axis=0)
+    chk.compare(H0, merged, sh.n_q_heads, sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma, 0, 3, commit=True)
+
+
+def test_default_window_start_is_trailing_window(gpu, chk):
+    """win_start = NULL means h = seq_len - W (t = 0)."""
+    wl = kin.generate(kin.scaled(kin.CFG1, n_seqs=3, hist_lo=16, hist_hi=200), seed=12)
+    _parity(gpu, chk, wl, use_win_start=False)
+
+
+def test_buffer_only_queries_flag(gpu, oracle):
+    """KARA_SCORE_QBUF_ONLY: the 'w/o Bi-Attention' ablation scores with the buffer's queries."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_seqs=2, n_q_heads=4, n_kv_heads=2, hist_lo=20, hist_hi=60), seed=13)
+    sh = wl.shape
+    out, _, _ = gu.gpu_compress(wl, flags=kara.KARA_KEEP_DEBUG | kara.KARA_SCORE_QBUF_ONLY)
+    from oracle import check
+    H = check.host_image(wl)
+    for s in range(2):
+        h = int(H["ws"][s])
+        pos = np.arange(h, h + sh.n)
+        for hk in range(2):
+            krows = H["k"][0, H["bt"][s, pos // 16], hk, pos % 16]
+            q = np.ascontiguousarray(H["q"][0, s][:, hk * sh.G:(hk + 1) * sh.G])
+            A64, _ = oracle.scores(q, np.ascontiguousarray(krows), buffer_only_U=sh.U)
+            tol = check.score_tolerance(A64, sh.G, sh.U, sh.n)
+            assert (np.abs(out["scores"][0, s, hk] - A64) <= tol).all()
+
+
+def test_device_status_word_flags_bad_inputs(gpu):
+    kara, gu = gpu
+    wl = kin.generate(kin.CFG1, seed=1)
+    D = gu.to_cuda(wl)
+    D["bt"][0, 17] = wl.num_blocks + 5          # a window block outside the pool
+    out, cache, _ = gu.gpu_compress(wl, dev_tensors=D, flags=kara.KARA_KEEP_DEBUG)
+    assert out["status"] & kara.KARA_ST_BAD_BLOCK
+    D = gu.to_cuda(wl)
+    D["sl"][0] = 40                              # shorter than its window
+    out, cache, _ = gu.gpu_compress(wl, dev_tensors=D, flags=kara.KARA_KEEP_DEBUG, use_win_start=False)
+    assert out["status"] & kara.KARA_ST_SHORT_SEQ
+
+
+def test_argument_errors_are_reported_not_thrown(gpu):
+    kara, gu = gpu
+    wl = kin.generate(kin.CFG1, seed=1)
+    with pytest.raises(kara.KaraError) as e:
+        gu.gpu_compress(wl, overrides=dict(alpha=12))      # keep - alpha = 0
+    assert e.value.code == kara.KARA_EBUDGET
+    with pytest.raises(kara.KaraError) as e:
+        gu.gpu_compress(wl, overrides=dict(gamma=2))
+    assert e.value.code == kara.KARA_EBUDGET
+
+
+def test_host_buffer_entry_point(gpu, chk):
+    """kara_compress_window_host: host tables / queries in, same result as the device call."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_seqs=3, hist_lo=20, hist_hi=90), seed=21)
+    sh = wl.shape
+    ref, _, _ = gu.gpu_compress(wl)
+    D = gu.to_cuda(wl)
+    cache = kara.KaraCache(sh.block_size, 1, sh.n_kv_heads, sh.head_dim)
+    cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+    bt, sl, ws = wl.block_table.clone().pin_memory(), wl.seq_lens.clone().pin_memory(), wl.win_start.clone().pin_memory()
+    q = wl.window_q.clone().pin_memory()
+    nfree = cache.compress_window_host(0, 1, bt, sl, ws, q, sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma)
+    np.testing.assert_array_equal(bt.numpy(), ref["bt"])
+    np.testing.assert_array_equal(sl.numpy(), ref["sl"])
+    assert nfree == int(ref["fc"][0])
+    np.testing.assert_array_equal(gu.bits(D["k"]), ref["k"])
+    np.testing.assert_array_equal(gu.bits(D["v"]), ref["v"])
+
+
+def test_gather_debug_logical_rows(gpu):
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_seqs=2, hist_lo=20, hist_hi=60), seed=31)
+    D = gu.to_cuda(wl)
+    cache = kara.KaraCache(16, 1, 1, 64)
+    cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+    for s in range(2):
+        ln = int(wl.seq_lens[s])
+        for what, pool in ((kara.KARA_DBG_K_LOGICAL, wl.k_pool), (kara.KARA_DBG_V_LOGICAL, wl.v_pool)):
+            got = cache.gather_debug(what, 0, s, 0, D["bt"], D["sl"])
+            ref = gu.bits(kin.logical_rows(pool, 0, wl.block_table[s], ln, 0))
+            np.testing.assert_array_equal(got, ref)
+    fl = cache.gather_debug(kara.KARA_DBG_FREE_LIST, 0, 0, 0)
+    np.testing.assert_array_equal(fl, wl.free_list[: int(wl.free_count)].numpy())
