@@ -55,7 +55,7 @@ def _parity(gpu, chk, wl, flags_extra=0, overrides=None, lb=None, le=None, use_w
 def test_cfg1_tiny(gpu, chk, seed):
     """BASELINE.json configs[0]: 1 seq, 1 layer, GQA 4/1, d=64, bs=16, h=256, W=64, r=20 %."""
     stats, out, _ = _parity(gpu, chk, kin.generate(kin.CFG1, seed=seed))
-    assert stats["keep"] == 12 and stats["s3_hard_mismatch"] == 0
+    assert stats["keep"] == 12 and stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
     # the planted keys are retained
     wl = kin.generate(kin.CFG1, seed=seed)
     planted = set(np.flatnonzero(wl.salient[0].numpy()).tolist())
@@ -70,7 +70,8 @@ def test_cfg2_shape_two_layers(gpu, chk, simt):
     wl = kin.generate(kin.scaled(kin.CFG2, n_layers=2, hist_lo=4099, hist_hi=4099), seed=2)
     stats, out, _ = _parity(gpu, chk, wl, flags_extra=kara.KARA_SCORE_SIMT if simt else 0)
     assert stats["keep"] == 96
-    assert stats["score_path"] == (1 if simt else stats["score_path"])
+    # the default path on a B200 is the tcgen05/TMA kernel; KARA_SCORE_SIMT forces the CUDA-core one
+    assert stats["score_path"] == (1 if simt else 2)
     assert out["sl"][0] == 4099 + 96 + 32
     assert int(out["fc"][0]) - int(wl.free_count[0]) == math.ceil((4099 + 512) / 16) - math.ceil((4099 + 128) / 16)
 
