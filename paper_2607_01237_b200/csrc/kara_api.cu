@@ -64,9 +64,11 @@ int budget(int n, double ratio) {
   return (int)std::ceil(ratio * (double)n - 1e-9);   // reading G5
 }
 
-WsLayout ws_layout(int units, int n, int k, int keep) {
+// tiles_per_unit: query tiles of 128 rows x one head (full-window queries: an upper bound for
+// KARA_SCORE_QBUF_ONLY, whose strip count has the same bound because T shrinks with tpu)
+WsLayout ws_layout(int units, int n, int k, int keep, int tiles_per_unit) {
   WsLayout w{};
-  w.parts = kMaxParts;
+  w.parts = strips_bound(units, tiles_per_unit);
   w.n_pad = round_up(n, 4);
   w.k_pad = round_up(k > 0 ? k : 1, 4);
   w.keep_pad = round_up(keep > 0 ? keep : 1, 4);
@@ -178,13 +180,14 @@ int kara_attach_pool(kara_cache* c, void* k_pool, void* v_pool, int64_t num_bloc
 
 size_t kara_workspace_bytes(const kara_cache* c, int n_layers_in_call, int n_seqs, int n_q_heads, int W, int U,
                             double ratio, int alpha) {
-  (void)n_q_heads;
-  if (!c || n_layers_in_call <= 0 || n_seqs <= 0 || U < 0 || W <= U) return 0;
+  if (!c || n_layers_in_call <= 0 || n_seqs <= 0 || U < 0 || W <= U || n_q_heads <= 0 ||
+      n_q_heads % c->g.n_kv_heads != 0)
+    return 0;
   const int n = W - U;
   const int keep = budget(n, ratio);
   if (keep < 0) return 0;
   const int units = n_layers_in_call * n_seqs * c->g.n_kv_heads;
-  return ws_layout(units, n, keep - alpha, keep).total;
+  return ws_layout(units, n, keep - alpha, keep, (W + 127) / 128 * (n_q_heads / c->g.n_kv_heads)).total;
 }
 
 int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_seqs, int32_t* block_table,
@@ -204,7 +207,7 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   const int nL = layer_end - layer_begin;
   const int n = W - U;
   const int units = nL * n_seqs * c->g.n_kv_heads;
-  const WsLayout w = ws_layout(units, n, keep - alpha, keep);
+  const WsLayout w = ws_layout(units, n, keep - alpha, keep, (W + 127) / 128 * (n_q_heads / c->g.n_kv_heads));
   if (workspace_bytes < w.total)
     return fail(KARA_ENOMEM, "workspace %zu bytes < %zu needed", workspace_bytes, w.total);
 
@@ -235,6 +238,8 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   k.idx_topk = reinterpret_cast<int32_t*>(base + w.topk_off);
   k.idx_final = reinterpret_cast<int32_t*>(base + w.final_off);
   k.n_pad = w.n_pad; k.k_pad = w.k_pad; k.keep_pad = w.keep_pad;
+  k.parts = w.parts;          // strips reserved per unit; the score kernels say how many they fill
+  k.part_T = k.part_nc = k.part_tpu = 0;
   k.keep_debug = (flags & KARA_KEEP_DEBUG) ? 1 : 0;
   k.free_list = c->free_list;
   k.free_count = c->free_count;
@@ -250,13 +255,15 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   }
   if (use_tc) {
     int nl = 0;
-    rc = score_tc_launch(&c->tc, k, st, &nl);   // sets k.parts
+    rc = score_tc_launch(&c->tc, k, st, &nl);   // sets k.part_T / part_nc / part_tpu
     if (rc != KARA_OK) return fail(rc, "score_tc_launch: %s", score_tc_error());
     launches += nl;
     c->last_score_path = 2;
   } else {
     const int rows = (W - k.q_row_begin) * k.G;
-    k.parts = rows >= 128 * kMaxParts ? kMaxParts : (rows + 127) / 128;
+    const int want = (rows + 127) / 128;
+    k.parts = want < w.parts ? want : w.parts;   // row parts of the SIMT kernel, all of them filled
+    if (k.parts > 16) k.parts = 16;
     KARA_CUDA(launch_score_simt(k, st));
     ++launches;
     c->last_score_path = 1;

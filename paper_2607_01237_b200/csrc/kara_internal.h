@@ -31,11 +31,16 @@ struct Call {
   const __nv_bfloat16* window_q;
   // workspace pieces
   int32_t* status;   // [8]
-  float* partial;    // [units][parts][n_pad]
+  float* partial;    // [units][parts][n_pad]  (parts = strips reserved per unit)
   float* scores;     // [units][n_pad]
   int32_t* idx_topk; // [units][k_pad]
   int32_t* idx_final;// [units][keep_pad]
   int parts, n_pad, k_pad, keep_pad;
+  // Which strips of a unit hold data.  part_T == 0: all `parts` strips (SIMT kernel).  part_T > 0
+  // (tcgen05 kernel): the T = units*part_tpu query tiles are split into part_nc contiguous ranges,
+  // one per cluster; a unit's tiles touch clusters [tile_owner(first), tile_owner(last)] and each
+  // of them writes two strips (one per softmax warpgroup): strips_of_unit().
+  int part_T, part_nc, part_tpu;
   int keep_debug;
   int32_t* free_list;
   int32_t* free_count;
@@ -46,10 +51,32 @@ struct WsLayout {
   int parts, n_pad, k_pad, keep_pad;
 };
 
-constexpr int kMaxParts = 16;   // partial column sums per unit, reduced in fixed order by select
+constexpr int kMaxSms = 160;    // upper bound on clusters of one launch (B200: 148 SMs)
 constexpr int kMaxN = 2048;     // largest compressible region (cfg 5: 1984)
 
 inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// Cluster that owns global query tile `tile` when T tiles are cut into nc contiguous ranges
+// [floor(c T / nc), floor((c+1) T / nc)).
+__host__ __device__ inline int tile_owner(long long tile, int nc, int T) {
+  return (int)(((tile + 1) * nc - 1) / T);
+}
+// Number of partial-score strips the score kernel wrote for `unit` (see Call::part_T).
+__host__ __device__ inline int strips_of_unit(int unit, int parts, int part_T, int part_nc, int part_tpu) {
+  if (part_T <= 0) return parts;
+  const long long first = (long long)unit * part_tpu;
+  return 2 * (tile_owner(first + part_tpu - 1, part_nc, part_T) - tile_owner(first, part_nc, part_T) + 1);
+}
+// Upper bound of strips_of_unit over every split of units*tpu tiles into <= kMaxSms ranges: a
+// range holds >= p = floor(T/nc) tiles, so the tpu consecutive tiles of a unit meet at most
+// ceil((tpu-1)/p) + 1 ranges, and never more than tpu.
+inline int strips_bound(int units, int tpu) {
+  long long p = ((long long)units * tpu) / kMaxSms;
+  if (p < 1) p = 1;
+  long long ranges = (tpu - 1 + p - 1) / p + 1;
+  if (ranges > tpu) ranges = tpu;
+  return (int)(2 * ranges);
+}
 
 // unit index -> (layer-in-call, sequence, kv head)
 __host__ __device__ inline void unit_decode(int unit, int n_seqs, int n_kv_heads, int& li, int& s, int& hk) {

@@ -2,26 +2,35 @@
 // 5th-generation tensor cores of sm_100a: TMA -> shared memory, tcgen05.mma -> TMEM, softmax out
 // of TMEM, deterministic column sums.  DESIGN.md §Kernels/a1 has the derivation of every choice.
 //
-// Decomposition.  A work item is (unit, part): a unit is one (layer, sequence, KV head); a part is
-// a contiguous range of the unit's query tiles; a query tile is 128 window tokens x ONE query
-// head of the GQA group (rows of a row-softmax are independent, so any (token, head) -> row map
-// is valid; TMA reads the rows at stride n_q_heads*d).  A thread-block cluster of CL CTAs owns an
-// item; CTA r of the cluster owns the 256 key rows [256 r, 256 r + 256) of the block-aligned key
-// panel (whole paged blocks are loaded, one TMA box per block and 64-element column panel; rows
-// outside the compressible region [h, h+n) are masked to -inf).  Per tile and CTA:
+// Decomposition.  A unit is one (layer, sequence, KV head).  A query tile is 128 window tokens x
+// ONE query head of the GQA group (rows of a row-softmax are independent, so any (token, head) ->
+// row map is valid; TMA reads the rows at stride n_q_heads*d).  All T = units * tiles_per_unit
+// tiles of the launch form one sequence that is cut into n_clusters contiguous, equally long
+// ranges (perfect balance; a range crosses unit boundaries, the part of a unit inside a range is
+// a "segment").  A thread-block cluster of CL CTAs owns a range; CTA r of the cluster owns the
+// 256 key rows [256 r, 256 r + 256) of the block-aligned key panel (whole paged blocks are
+// loaded, one TMA box per block and 64-element column panel; rows outside the compressible
+// region [h, h+n) are masked to -inf).  Per tile and CTA:
 //   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM
-//   m_i^r = max_j S_ij ;  e_ij = exp2((S_ij - m_i^r) c) (stored back to TMEM) ;  l_i^r = sum_j e_ij
-//   (m^r, l^r) of the 128 rows are exchanged across the cluster through distributed shared memory:
-//       m_i = max_r m_i^r ;  l_i = sum_r l_i^r exp2((m_i^r - m_i) c) ;  w_i^r = exp2((m_i^r - m_i) c) / l_i
-//   acc_j += sum_i e_ij w_i^r     per-thread registers: with the 16x256b TMEM load shape a thread
-//                                 holds 4 rows x 1/4 of the columns, so the column sum over ALL
-//                                 tiles of the item is a plain FFMA; lanes are combined once per item.
-// TMEM holds two 128 x 256 fp32 S buffers (all 512 columns): the MMA of tile t+1 runs while the
-// softmax warpgroup of tile t is still reading; two softmax warpgroups alternate tiles.
+//   pass B (one TMEM read, one write):  a thread holds 4 rows x 16 columns of a 64-column chunk;
+//       it shifts by ITS OWN maximum of those 16 logits, rounded to an integer z (log2 domain):
+//       e = exp2(s c - z), written back in place; l += e.  No separate max pass, no shuffles.
+//   statistics: z and l of the (<= 4) chunks, the 4 lanes of a row and the CL CTAs of the
+//       cluster are merged with exact power-of-two rescaling built by integer arithmetic (no
+//       MUFU); across CTAs through distributed shared memory with st.async + a transaction-count
+//       mbarrier per warp (no fence, no cluster barrier).  w_(row,chunk) = 2^(z - Z_row) / L_row.
+//   pass C (one TMEM read):  acc_j += sum_i e_ij w_i   per-thread registers: with the 16x256b
+//       TMEM load shape the column sum over ALL tiles of a segment is a plain packed FFMA2;
+//       lanes are combined once per segment.
+// TMEM holds two 128 x 256 fp32 S buffers (all 512 columns): the MMA of the next tile of a
+// warpgroup runs while the other warpgroup is in its softmax; two softmax warpgroups alternate
+// tiles.  The K panel is double-buffered so a segment change costs no bubble.
 //
-// Warp roles (320 threads): warps 0-3 softmax WG0, 4-7 softmax WG1, 8 TMA producer, 9 MMA issuer.
-// Output: partial[unit][part][j] (fp32), summed over parts in fixed order by the select kernel, so
-// scores are bit-reproducible run to run (no atomics anywhere).
+// Warp roles (384 threads): warps 0-3 softmax WG0, 4-7 softmax WG1, 8 TMA producer, 9 MMA issuer,
+// 10-11 idle (they exist so that setmaxnreg can move their registers to the softmax warpgroups).
+// Output: partial[unit][2 p + wg][j] (fp32), p = index of the range among those that touch the
+// unit; the select kernel sums the strips in fixed order, so scores are bit-reproducible run to
+// run (no atomics anywhere).
 #include <cuda.h>
 
 #include <cstdio>
@@ -36,12 +45,17 @@ namespace {
 constexpr int kSoftmaxWarps = 8;
 constexpr int kProducerWarp = 8;
 constexpr int kMmaWarp = 9;
-constexpr int kThreads = 32 * 10;
+constexpr int kThreads = 32 * 12;             // 3 warpgroups (setmaxnreg works per warpgroup); warps 10, 11 idle
+constexpr int kRegsSoftmax = 232, kRegsOther = 40;   // 168 x 384 at launch -> 2 x 128 x 232 + 128 x 40
 constexpr int kTileM = 128;
 constexpr int kKeysPerCta = 256;
-constexpr int kQStages = 3;
+constexpr int kQStages = 2;
 constexpr int kTmemCols = 512;
+constexpr float kZLim = 32000.f;              // integer shifts z are clamped to +-kZLim (|logit| log2e / sqrt(d) beyond that is not served)
+constexpr uint32_t kZEmptyPair = 0x83008300u; // two int16 -32000: the shift of a piece with no valid key
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kMagic = 12582912.f;          // 1.5 * 2^23: x + kMagic rounds x to an integer in the low mantissa bits
+constexpr int kMagicBits = 0x4B400000;
 
 char g_tc_err[256] = "";
 
@@ -72,26 +86,15 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "KARA_DONE_%=:\n\t}"
       :: "r"(bar), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "KARA_WAITC_%=:\n\t"
-      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra KARA_DONEC_%=;\n\t"
-      "bra KARA_WAITC_%=;\n\t"
-      "KARA_DONEC_%=:\n\t}"
-      :: "r"(bar), "r"(parity) : "memory");
-}
 __device__ __forceinline__ uint32_t mapa(uint32_t local_addr, uint32_t cta) {
   uint32_t r;
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta));
   return r;
 }
-__device__ __forceinline__ void st_cluster_f2(uint32_t addr, float a, float b) {
-  asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" :: "r"(addr), "f"(a), "f"(b) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(cluster_addr) : "memory");
+// 8-byte store into a peer CTA's shared memory that signals the peer's mbarrier (complete_tx)
+__device__ __forceinline__ void st_async_b32x2(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t cluster_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b32 [%0], {%1, %2}, [%3];"
+               :: "r"(cluster_addr), "r"(a), "r"(b), "r"(cluster_bar) : "memory");
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -145,38 +148,33 @@ __device__ __forceinline__ uint32_t make_idesc_bf16(int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 }
 
-#define KARA_TMEM_REGS32(r, o)                                                                       \
-  "=r"(r[o + 0]), "=r"(r[o + 1]), "=r"(r[o + 2]), "=r"(r[o + 3]), "=r"(r[o + 4]), "=r"(r[o + 5]),    \
-  "=r"(r[o + 6]), "=r"(r[o + 7]), "=r"(r[o + 8]), "=r"(r[o + 9]), "=r"(r[o + 10]), "=r"(r[o + 11]),  \
-  "=r"(r[o + 12]), "=r"(r[o + 13]), "=r"(r[o + 14]), "=r"(r[o + 15]), "=r"(r[o + 16]), "=r"(r[o + 17]), \
-  "=r"(r[o + 18]), "=r"(r[o + 19]), "=r"(r[o + 20]), "=r"(r[o + 21]), "=r"(r[o + 22]), "=r"(r[o + 23]), \
-  "=r"(r[o + 24]), "=r"(r[o + 25]), "=r"(r[o + 26]), "=r"(r[o + 27]), "=r"(r[o + 28]), "=r"(r[o + 29]), \
-  "=r"(r[o + 30]), "=r"(r[o + 31])
-#define KARA_TMEM_IN32(r, o)                                                                         \
-  "r"(r[o + 0]), "r"(r[o + 1]), "r"(r[o + 2]), "r"(r[o + 3]), "r"(r[o + 4]), "r"(r[o + 5]),          \
-  "r"(r[o + 6]), "r"(r[o + 7]), "r"(r[o + 8]), "r"(r[o + 9]), "r"(r[o + 10]), "r"(r[o + 11]),        \
-  "r"(r[o + 12]), "r"(r[o + 13]), "r"(r[o + 14]), "r"(r[o + 15]), "r"(r[o + 16]), "r"(r[o + 17]),    \
-  "r"(r[o + 18]), "r"(r[o + 19]), "r"(r[o + 20]), "r"(r[o + 21]), "r"(r[o + 22]), "r"(r[o + 23]),    \
-  "r"(r[o + 24]), "r"(r[o + 25]), "r"(r[o + 26]), "r"(r[o + 27]), "r"(r[o + 28]), "r"(r[o + 29]),    \
-  "r"(r[o + 30]), "r"(r[o + 31])
+#define KARA_TMEM_REGS32(r)                                                                          \
+  "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),    \
+  "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]),           \
+  "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]),         \
+  "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]),         \
+  "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+#define KARA_TMEM_IN32(r)                                                                            \
+  "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),            \
+  "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),      \
+  "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),    \
+  "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
 
 // 16 lanes x 64 columns: thread t gets, for column group i (8 columns), regs 4i+{0,1} = lane t/4,
 // columns 8i + 2(t%4) + {0,1}; regs 4i+{2,3} = lane t/4 + 8, same columns.
-template <int O>
-__device__ __forceinline__ void tmem_ld_16x256b_x8(uint32_t taddr, uint32_t (&r)[64]) {
+__device__ __forceinline__ void tmem_ld_16x256b_x8(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.16x256b.x8.b32 "
       "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
       "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-      : KARA_TMEM_REGS32(r, O) : "r"(taddr) : "memory");
+      : KARA_TMEM_REGS32(r) : "r"(taddr) : "memory");
 }
-template <int O>
-__device__ __forceinline__ void tmem_st_16x256b_x8(uint32_t taddr, const uint32_t (&r)[64]) {
+__device__ __forceinline__ void tmem_st_16x256b_x8(uint32_t taddr, const uint32_t (&r)[32]) {
   asm volatile(
       "tcgen05.st.sync.aligned.16x256b.x8.b32 [%32], "
       "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
       "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
-      :: KARA_TMEM_IN32(r, O), "r"(taddr) : "memory");
+      :: KARA_TMEM_IN32(r), "r"(taddr) : "memory");
 }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
@@ -186,6 +184,37 @@ __device__ __forceinline__ float ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float y;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
+  return y;
+}
+// packed fp32 pairs (FFMA2 / FADD2 on sm_100)
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ uint64_t pk2u(uint32_t lo, uint32_t hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+// 2^d for d <= 0 built from the exponent field; 0 for d <= -127 (such weights are below fp32's range)
+__device__ __forceinline__ float pow2i(int d) { return __int_as_float(max(d + 127, 0) << 23); }
 
 // ------------------------------------------------------------------------------------------------
 // shared-memory carve-up (dynamic smem, manually aligned to 1024 B for the 128B swizzle)
@@ -193,33 +222,38 @@ __device__ __forceinline__ float ex2(float x) {
 template <int D, int CL>
 struct Smem {
   static constexpr int kPanels = D / 64;
+  static constexpr int kKStages = CL >= 8 ? 1 : 2;   // 8-CTA clusters need the room for the exchange slots
   static constexpr int kKBytes = kPanels * kKeysPerCta * 128;
   static constexpr int kQStageBytes = kPanels * kTileM * 128;
   static constexpr int kOffK = 0;
-  static constexpr int kOffQ = kOffK + kKBytes;
-  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;        // float [8][256]
-  static constexpr int kOffXch = kOffColsum + kSoftmaxWarps * kKeysPerCta * 4;  // float2 [4][CL][128]
-  static constexpr int kOffBars = kOffXch + 4 * CL * kTileM * 8;
-  // barriers: qfull[3] qempty[3] kfull kempty tfull[2] tempty[2] xbar[4]  = 16 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 16 * 8;
+  static constexpr int kOffQ = kOffK + kKStages * kKBytes;
+  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;            // float [8][256]
+  static constexpr int kOffXch = kOffColsum + kSoftmaxWarps * kKeysPerCta * 4;  // uint2 [8 warps][2][CL][32]
+  static constexpr int kOffBars = kOffXch + kSoftmaxWarps * 2 * CL * 32 * 8;
+  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2] tempty[2] xbar[8][2]  = 28 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 28 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
 
-struct ItemInfo {
+// One segment: the tiles [t0, t1) of `unit` that fall into this cluster's range.
+struct Seg {
   int unit, part, li, s, hk, layer;
   int h, fb, off;          // window start, first key block (table index), h - fb*bs
   int c_lo, c_hi;          // this CTA's valid key columns [c_lo, c_hi) within its 256
   int n_cols;              // MMA N for this CTA: valid columns rounded up to 16 (>= 16)
-  int t0, t1;              // tile range of the part
+  int t0, t1;
   bool ok;
 };
 
-template <int CL>
-__device__ __forceinline__ ItemInfo decode_item(const Call& c, int item, int rank, int tiles_per_unit, int tiles_per_part) {
-  ItemInfo it;
-  it.unit = item / c.parts;
-  it.part = item % c.parts;
+__device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long g_end, int rank, int cluster_id,
+                                          int n_clusters, int T, int tpu) {
+  Seg it;
+  it.unit = (int)(g / tpu);
+  it.t0 = (int)(g - (long long)it.unit * tpu);
+  const long long left = g_end - g;
+  it.t1 = (int)(left < (long long)(tpu - it.t0) ? it.t0 + left : tpu);
+  it.part = cluster_id - tile_owner((long long)it.unit * tpu, n_clusters, T);
   unit_decode(it.unit, c.n_seqs, c.g.n_kv_heads, it.li, it.s, it.hk);
   it.layer = c.layer_begin + it.li;
   const int len = c.seq_lens[it.s];
@@ -235,9 +269,77 @@ __device__ __forceinline__ ItemInfo decode_item(const Call& c, int item, int ran
   it.c_hi = min(max(hi, 0), kKeysPerCta);
   if (!it.ok) it.c_lo = it.c_hi = 0;
   it.n_cols = max(16, (it.c_hi + 15) & ~15);
-  it.t0 = min(tiles_per_unit, it.part * tiles_per_part);
-  it.t1 = min(tiles_per_unit, it.t0 + tiles_per_part);
   return it;
+}
+
+// ---- pass B on one half-chunk: 2 rows (K0, K0+1) x 16 columns of chunk C held in r[32] ----------
+// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column 64 C + 8 i + 2 qd + j.
+// Online softmax with exact power-of-two rescaling: the shift of this (row, chunk) is the running
+// maximum z = max(z_run, round(m c)) of the thread's integer shifts (log2 domain), so e <= 2^0.5;
+// l_run is rescaled by 2^(z_old - z) built from the exponent field (no MUFU).  z is clamped to
+// [-kZLim, kZLim] and kept as int16 (zp); a fully masked piece has m = -inf -> z = -kZLim, e = 0.
+template <int C, int K0>
+__device__ __forceinline__ void pass_b_half(uint32_t (&r)[32], uint32_t (&zp)[4][2], int (&zrun)[4], float (&lrun)[4],
+                                            float cs, int qd, int c_lo, int c_hi) {
+  constexpr int cb = C * 64;
+  if (!(cb >= c_lo && cb + 64 <= c_hi)) {   // warp-uniform: only the ragged first / last chunk
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int col = cb + 8 * i + 2 * qd + j;
+        if (col < c_lo || col >= c_hi) { r[4 * i + j] = 0xff800000u; r[4 * i + 2 + j] = 0xff800000u; }
+      }
+    }
+  }
+#define KARA_F(x) __uint_as_float(r[x])
+  float m0 = max3(KARA_F(0), KARA_F(1), KARA_F(4)), m1 = max3(KARA_F(2), KARA_F(3), KARA_F(6));
+  float m0b = max3(KARA_F(5), KARA_F(8), KARA_F(9)), m1b = max3(KARA_F(7), KARA_F(10), KARA_F(11));
+  m0 = max3(m0, KARA_F(12), KARA_F(13));   m1 = max3(m1, KARA_F(14), KARA_F(15));
+  m0b = max3(m0b, KARA_F(16), KARA_F(17)); m1b = max3(m1b, KARA_F(18), KARA_F(19));
+  m0 = max3(m0, KARA_F(20), KARA_F(21));   m1 = max3(m1, KARA_F(22), KARA_F(23));
+  m0b = max3(m0b, KARA_F(24), KARA_F(25)); m1b = max3(m1b, KARA_F(26), KARA_F(27));
+  m0 = max3(m0, KARA_F(28), KARA_F(29));   m1 = max3(m1, KARA_F(30), KARA_F(31));
+  m0 = fmaxf(m0, m0b);                     m1 = fmaxf(m1, m1b);
+#undef KARA_F
+  const float t0 = fminf(fmaxf(m0 * cs, -kZLim), kZLim) + kMagic;   // integer in the low mantissa bits
+  const float t1 = fminf(fmaxf(m1 * cs, -kZLim), kZLim) + kMagic;
+  const int z0 = max(zrun[K0], __float_as_int(t0) - kMagicBits);
+  const int z1 = max(zrun[K0 + 1], __float_as_int(t1) - kMagicBits);
+  const float l0s = lrun[K0] * pow2i(zrun[K0] - z0), l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
+  zrun[K0] = z0; zrun[K0 + 1] = z1;
+  zp[C][K0 / 2] = ((uint32_t)z0 & 0xffffu) | ((uint32_t)z1 << 16);
+  const float nz0 = kMagic - __int_as_float(z0 + kMagicBits), nz1 = kMagic - __int_as_float(z1 + kMagicBits);
+  const uint64_t cs2 = pk2(cs, cs), nz0_2 = pk2(nz0, nz0), nz1_2 = pk2(nz1, nz1);
+  uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    float a, b;
+    upk2(fma2(pk2u(r[4 * i], r[4 * i + 1]), cs2, nz0_2), a, b);
+    a = ex2(a); b = ex2(b);
+    l0 = add2(l0, pk2(a, b));
+    r[4 * i] = __float_as_uint(a); r[4 * i + 1] = __float_as_uint(b);
+    upk2(fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), cs2, nz1_2), a, b);
+    a = ex2(a); b = ex2(b);
+    l1 = add2(l1, pk2(a, b));
+    r[4 * i + 2] = __float_as_uint(a); r[4 * i + 3] = __float_as_uint(b);
+  }
+  float a, b;
+  upk2(l0, a, b); lrun[K0] = a + b;
+  upk2(l1, a, b); lrun[K0 + 1] = a + b;
+}
+
+// ---- pass C on one half-chunk: acc[C*8 + i] (columns 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------
+template <int C, int K0>
+__device__ __forceinline__ void pass_c_half(const uint32_t (&r)[32], uint64_t (&acc)[32], const float (&w)[4][4]) {
+  const uint64_t w0 = pk2(w[C][K0], w[C][K0]), w1 = pk2(w[C][K0 + 1], w[C][K0 + 1]);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    uint64_t a = acc[C * 8 + i];
+    a = fma2(pk2u(r[4 * i], r[4 * i + 1]), w0, a);
+    a = fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), w1, a);
+    acc[C * 8 + i] = a;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -246,7 +348,7 @@ __device__ __forceinline__ ItemInfo decode_item(const Call& c, int item, int ran
 template <int D, int CL>
 __global__ void __launch_bounds__(kThreads, 1)
 score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant__ CUtensorMap q_map,
-                const Call c, int n_items, int tiles_per_unit, int tiles_per_part, int tok_tiles) {
+                const Call c, int T, int tpu, int tok_tiles) {
   using SM = Smem<D, CL>;
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
@@ -255,22 +357,25 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t sK = base + SM::kOffK;
   const uint32_t sQ = base + SM::kOffQ;
   float* colsum = reinterpret_cast<float*>(gbase + SM::kOffColsum);
-  float2* xch = reinterpret_cast<float2*>(gbase + SM::kOffXch);
+  uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
-  const uint32_t qfull = bars, qempty = bars + 24, kfull = bars + 48, kempty = bars + 56;
+  const uint32_t qfull = bars, qempty = bars + 16, kfull = bars + 32, kempty = bars + 48;
   const uint32_t tfull = bars + 64, tempty = bars + 80, xbar = bars + 96;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rank = CL > 1 ? (int)cluster_ctarank() : 0;
   const int cluster_id = blockIdx.x / CL, n_clusters = gridDim.x / CL;
+  const long long g_begin = (long long)cluster_id * T / n_clusters;
+  const long long g_end = (long long)(cluster_id + 1) * T / n_clusters;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < kQStages; ++i) { mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1); }
-    mbar_init(kfull, 1);
-    mbar_init(kempty, 1);
-    for (int i = 0; i < 2; ++i) { mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 1); }
-    for (int i = 0; i < 4; ++i) mbar_init(xbar + 8 * i, 4 * CL);   // one arrive per softmax warp per CTA
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1);
+      mbar_init(kfull + 8 * i, 1); mbar_init(kempty + 8 * i, 1);
+      mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 4);   // one arrive per warp of the warpgroup
+    }
+    for (int i = 0; i < 16; ++i) mbar_init(xbar + 8 * i, 1);       // per softmax warp and parity
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
@@ -280,23 +385,31 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   if (CL > 1) cluster_sync_all();
   const uint32_t tmem_base = *tmem_ptr;
 
+  if (warp >= kSoftmaxWarps) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsOther));
   if (warp == kProducerWarp) {
     // ================================ TMA producer ==============================================
-    int q_iter = 0, k_iter = 0;
     const int blocks_per_cta = kKeysPerCta >> c.g.bs_log2;   // <= 16: one block per lane
-    for (int item = cluster_id; item < n_items; item += n_clusters) {
-      const ItemInfo it = decode_item<CL>(c, item, rank, tiles_per_unit, tiles_per_part);
-      if (!it.ok || it.t0 >= it.t1) continue;
-      // ---- K panel of this CTA: whole blocks, skipped if they hold no compressible key ----
-      mbar_wait(kempty, (k_iter & 1) ^ 1);
+    int q_iter = 0, k_iter = 0;
+    long long g = g_begin;
+    auto next_ok = [&](Seg& it) -> bool {
+      while (g < g_end) {
+        it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+        g += it.t1 - it.t0;
+        if (it.ok) return true;
+      }
+      return false;
+    };
+    // K panel of this CTA: whole blocks, skipped if they hold no compressible key
+    auto load_k = [&](const Seg& it) {
+      const int stage = k_iter % SM::kKStages, use = k_iter / SM::kKStages;
       ++k_iter;
-      int my_bytes = 0;
-      int my_blk = -1, my_row = 0;
+      mbar_wait(kempty + 8 * stage, (use & 1) ^ 1);
+      int my_bytes = 0, my_blk = -1, my_row = 0;
       if (lane < blocks_per_cta) {
-        const int lb = lane;
-        const int row0 = lb << c.g.bs_log2;                       // first panel row of this block in the CTA
+        const int row0 = lane << c.g.bs_log2;                     // first panel row of this block in the CTA
         if (row0 < it.c_hi && row0 + c.g.bs > it.c_lo) {          // block intersects the valid columns
-          const int tbl = it.fb + rank * blocks_per_cta + lb;
+          const int tbl = it.fb + rank * blocks_per_cta + lane;
           if (tbl < c.max_blocks) {
             const int b = c.block_table[(long long)it.s * c.max_blocks + tbl];
             if (b >= 0 && b < c.g.num_blocks) { my_blk = b; my_row = row0; my_bytes = c.g.bs * D * 2; }
@@ -307,39 +420,53 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       int tot = my_bytes;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-      if (lane == 0) mbar_expect_tx(kfull, (uint32_t)tot);
+      if (lane == 0) mbar_expect_tx(kfull + 8 * stage, (uint32_t)tot);
       __syncwarp();
       if (my_blk >= 0) {
         const long long grow = (((long long)it.layer * c.g.num_blocks + my_blk) * c.g.n_kv_heads + it.hk) << c.g.bs_log2;
 #pragma unroll
         for (int p = 0; p < SM::kPanels; ++p)
-          tma_load_2d(sK + p * (kKeysPerCta * 128) + my_row * 128, &k_map, kfull, p * 64, (int)grow);
+          tma_load_2d(sK + stage * SM::kKBytes + p * (kKeysPerCta * 128) + my_row * 128, &k_map, kfull + 8 * stage,
+                      p * 64, (int)grow);
       }
-      // ---- Q tiles ----
+      __syncwarp();
+    };
+    Seg cur, nxt;
+    bool have = next_ok(cur);
+    if (have) load_k(cur);
+    while (have) {
+      const bool have_n = next_ok(nxt);
+      if (SM::kKStages == 2 && have_n) load_k(nxt);     // prefetch: its stage was released by the segment before `cur`
       if (lane == 0) {
-        for (int tile = it.t0; tile < it.t1; ++tile, ++q_iter) {
+        for (int tile = cur.t0; tile < cur.t1; ++tile, ++q_iter) {
           const int stage = q_iter % kQStages, use = q_iter / kQStages;
           mbar_wait(qempty + 8 * stage, (use & 1) ^ 1);
           mbar_expect_tx(qfull + 8 * stage, SM::kQStageBytes);
-          const int g = tile / tok_tiles, tt = tile % tok_tiles;
-          const int tok = (it.li * c.n_seqs + it.s) * c.W + c.q_row_begin + tt * kTileM;
+          const int gq = tile / tok_tiles, tt = tile % tok_tiles;
+          const int tok = (cur.li * c.n_seqs + cur.s) * c.W + c.q_row_begin + tt * kTileM;
 #pragma unroll
           for (int p = 0; p < SM::kPanels; ++p)
             tma_load_3d(sQ + stage * SM::kQStageBytes + p * (kTileM * 128), &q_map, qfull + 8 * stage,
-                        p * 64, it.hk * c.G + g, tok);
+                        p * 64, cur.hk * c.G + gq, tok);
         }
       }
       __syncwarp();
+      if (SM::kKStages == 1 && have_n) load_k(nxt);
+      cur = nxt;
+      have = have_n;
     }
   } else if (warp == kMmaWarp) {
     // ================================ MMA issuer ================================================
     int q_iter = 0, k_iter = 0, tile_iter = 0;
-    for (int item = cluster_id; item < n_items; item += n_clusters) {
-      const ItemInfo it = decode_item<CL>(c, item, rank, tiles_per_unit, tiles_per_part);
-      if (!it.ok || it.t0 >= it.t1) continue;
+    for (long long g = g_begin; g < g_end;) {
+      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+      g += it.t1 - it.t0;
+      if (!it.ok) continue;
       const uint32_t idesc = make_idesc_bf16(it.n_cols);
+      const int kstage = k_iter % SM::kKStages, kuse = k_iter / SM::kKStages;
+      ++k_iter;
       if (lane == 0) {
-        mbar_wait(kfull, k_iter & 1);
+        mbar_wait(kfull + 8 * kstage, kuse & 1);
         for (int tile = it.t0; tile < it.t1; ++tile, ++q_iter, ++tile_iter) {
           const int stage = q_iter % kQStages, quse = q_iter / kQStages;
           const int buf = tile_iter & 1, tuse = tile_iter >> 1;
@@ -352,209 +479,174 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks) {
               const uint64_t ad = make_sw128_desc(sQ + stage * SM::kQStageBytes + p * (kTileM * 128) + ks * 32);
-              const uint64_t bd = make_sw128_desc(sK + p * (kKeysPerCta * 128) + ks * 32);
+              const uint64_t bd = make_sw128_desc(sK + kstage * SM::kKBytes + p * (kKeysPerCta * 128) + ks * 32);
               umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
             }
           }
           umma_commit(qempty + 8 * stage);   // Q stage reusable once these MMAs have read it
           umma_commit(tfull + 8 * buf);      // S tile complete
         }
-        umma_commit(kempty);                 // K panel reusable
+        umma_commit(kempty + 8 * kstage);    // K stage reusable
+      } else {
+        const int nt = it.t1 - it.t0;
+        q_iter += nt; tile_iter += nt;
       }
-      ++k_iter;
       __syncwarp();
     }
+  }
   } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsSoftmax));
     // ================================ softmax warpgroups =========================================
     const int wg = warp >> 2, wq = warp & 3;
     const int qd = lane & 3, lr = lane >> 2;            // column pair within a group of 8; row within 8
     const float cs = kLog2e * rsqrtf((float)D);
-    const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
-    float acc[64];
+    const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + wg * kKeysPerCta;
+    const uint32_t taddr_hi = taddr + (16u << 16);
+    uint64_t acc[32];
 #pragma unroll
-    for (int a = 0; a < 64; ++a) acc[a] = 0.f;
-    int tile_iter = 0, my_tiles = 0;
-    for (int item = cluster_id; item < n_items; item += n_clusters) {
-      const ItemInfo it = decode_item<CL>(c, item, rank, tiles_per_unit, tiles_per_part);
-      float* out = c.partial + ((long long)it.unit * c.parts + it.part) * c.n_pad;
-      if (!it.ok || it.t0 >= it.t1) {
-        // skipped item: its strip of partial sums must still be defined (zeros)
-        if (rank == 0) for (int j = threadIdx.x; j < c.n_pad; j += 32 * kSoftmaxWarps) out[j] = 0.f;
+    for (int a = 0; a < 32; ++a) acc[a] = 0ull;
+    int tile_iter = 0, my_use = 0;
+    for (long long g = g_begin; g < g_end;) {
+      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+      g += it.t1 - it.t0;
+      float* out = c.partial + ((long long)it.unit * c.parts + 2 * it.part + wg) * c.n_pad;
+      if (!it.ok) {
+        // skipped unit: its strips must still be defined (zeros); the status word says why
+        if (rank == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
         continue;
       }
       const int n_chunks = (it.n_cols + 63) >> 6;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         if ((tile_iter & 1) != wg) continue;
-        const int buf = wg, use = my_tiles;
-        ++my_tiles;
-        const int tt = tile % tok_tiles;
-        const int tok0 = c.q_row_begin + tt * kTileM;
-        mbar_wait(tfull + 8 * buf, (tile_iter >> 1) & 1);
+        const int use = my_use++;
+        mbar_wait(tfull + 8 * wg, (tile_iter >> 1) & 1);
         tc_fence_after();
-        const uint32_t taddr = tmem_base + lane_base + buf * kKeysPerCta;
-        uint32_t r[64];
 
-        auto load_chunk = [&](int ch) {
-          tmem_ld_16x256b_x8<0>(taddr + ch * 64, r);
-          tmem_ld_16x256b_x8<32>(taddr + (16u << 16) + ch * 64, r);
-          tmem_wait_ld();
-        };
-        auto mask_chunk = [&](int ch) {
-          const int cb = ch * 64;
-          if (cb >= it.c_lo && cb + 64 <= it.c_hi) return;
+        // ---- pass B: e = 2^(s c - z) in place; z (int16 pairs) per (row, chunk), running (z, l) per row ----
+        uint32_t zp[4][2];
+        int zq[4];
+        float lq[4];
 #pragma unroll
-          for (int i = 0; i < 8; ++i) {
+        for (int k = 0; k < 4; ++k) { zq[k] = -(int)kZLim; lq[k] = 0.f; }
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              const int col = cb + 8 * i + 2 * qd + j;
-              const bool v = (col >= it.c_lo) && (col < it.c_hi);
-              if (!v) {
-                r[4 * i + j] = 0xff800000u; r[4 * i + 2 + j] = 0xff800000u;
-                r[32 + 4 * i + j] = 0xff800000u; r[32 + 4 * i + 2 + j] = 0xff800000u;
-              }
-            }
-          }
-        };
-
-        // ---- pass A: row maxima over this CTA's valid columns ----
-        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-        for (int ch = 0; ch < n_chunks; ++ch) {
-          load_chunk(ch);
-          mask_chunk(ch);
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            mx[0] = fmaxf(mx[0], fmaxf(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1])));
-            mx[1] = fmaxf(mx[1], fmaxf(__uint_as_float(r[4 * i + 2]), __uint_as_float(r[4 * i + 3])));
-            mx[2] = fmaxf(mx[2], fmaxf(__uint_as_float(r[32 + 4 * i]), __uint_as_float(r[32 + 4 * i + 1])));
-            mx[3] = fmaxf(mx[3], fmaxf(__uint_as_float(r[32 + 4 * i + 2]), __uint_as_float(r[32 + 4 * i + 3])));
-          }
+        for (int ch = 0; ch < 4; ++ch) { zp[ch][0] = zp[ch][1] = kZEmptyPair; }
+        uint32_t ra[32], rb[32];
+        tmem_ld_16x256b_x8(taddr, ra);
+#define KARA_PASS_B(CH)                                                                        \
+        if (CH < n_chunks) {                                                                   \
+          tmem_wait_ld();                                                                      \
+          tmem_ld_16x256b_x8(taddr_hi + CH * 64, rb);                                          \
+          pass_b_half<CH, 0>(ra, zp, zq, lq, cs, qd, it.c_lo, it.c_hi);                        \
+          tmem_st_16x256b_x8(taddr + CH * 64, ra);                                             \
+          tmem_wait_ld();                                                                      \
+          if (CH + 1 < n_chunks) tmem_ld_16x256b_x8(taddr + (CH + 1) * 64, ra);                \
+          pass_b_half<CH, 2>(rb, zp, zq, lq, cs, qd, it.c_lo, it.c_hi);                        \
+          tmem_st_16x256b_x8(taddr_hi + CH * 64, rb);                                          \
         }
-        float ms[4];   // local row max in the exp2 domain; 0 stands in for "no valid key in this CTA"
+        KARA_PASS_B(0) KARA_PASS_B(1) KARA_PASS_B(2) KARA_PASS_B(3)
+#undef KARA_PASS_B
+
+        // ---- row statistics: quad -> CTA, cluster -> row ----
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          mx[k] = fmaxf(mx[k], __shfl_xor_sync(0xffffffffu, mx[k], 1));
-          mx[k] = fmaxf(mx[k], __shfl_xor_sync(0xffffffffu, mx[k], 2));
-          ms[k] = (mx[k] == -INFINITY) ? 0.f : mx[k] * cs;
+          const int zt = zq[k];
+          int zz = max(zt, __shfl_xor_sync(0xffffffffu, zt, 1));
+          zz = max(zz, __shfl_xor_sync(0xffffffffu, zz, 2));
+          float lt = lq[k] * pow2i(zt - zz);
+          lt += __shfl_xor_sync(0xffffffffu, lt, 1);
+          lt += __shfl_xor_sync(0xffffffffu, lt, 2);
+          zq[k] = zz; lq[k] = lt;
         }
-        // ---- pass B: e = exp2(s c - m c), row sums, e written back in place ----
-        float ls[4] = {0.f, 0.f, 0.f, 0.f};
-        for (int ch = 0; ch < n_chunks; ++ch) {
-          load_chunk(ch);
-          mask_chunk(ch);
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              const float e0 = ex2(fmaf(__uint_as_float(r[4 * i + j]), cs, -ms[0]));
-              const float e1 = ex2(fmaf(__uint_as_float(r[4 * i + 2 + j]), cs, -ms[1]));
-              const float e2 = ex2(fmaf(__uint_as_float(r[32 + 4 * i + j]), cs, -ms[2]));
-              const float e3 = ex2(fmaf(__uint_as_float(r[32 + 4 * i + 2 + j]), cs, -ms[3]));
-              ls[0] += e0; ls[1] += e1; ls[2] += e2; ls[3] += e3;
-              r[4 * i + j] = __float_as_uint(e0); r[4 * i + 2 + j] = __float_as_uint(e1);
-              r[32 + 4 * i + j] = __float_as_uint(e2); r[32 + 4 * i + 2 + j] = __float_as_uint(e3);
-            }
-          }
-          tmem_st_16x256b_x8<0>(taddr + ch * 64, r);
-          tmem_st_16x256b_x8<32>(taddr + (16u << 16) + ch * 64, r);
-        }
-        tmem_wait_st();
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          ls[k] += __shfl_xor_sync(0xffffffffu, ls[k], 1);
-          ls[k] += __shfl_xor_sync(0xffffffffu, ls[k], 2);
-        }
-        // local "max" that is honest about emptiness for the exchange
-        float mloc[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) mloc[k] = (mx[k] == -INFINITY) ? -INFINITY : ms[k];
-
-        // ---- row weights w_i: cluster-wide softmax normalisation ----
-        float w[4];
+        int zf[4];
+        float inv[4];
         if (CL == 1) {
 #pragma unroll
-          for (int k = 0; k < 4; ++k) w[k] = ls[k] > 0.f ? 1.f / ls[k] : 0.f;
+          for (int k = 0; k < 4; ++k) { zf[k] = zq[k]; inv[k] = lq[k] > 0.f ? 1.f / lq[k] : 0.f; }
         } else {
-          const int slot = wg * 2 + (use & 1);
-          float2* my_slot = xch + (size_t)slot * CL * kTileM;
-          if (qd == 0) {
+          // lane (lr, qd) publishes row lr + 8 qd of this warp to every peer CTA
+          const int pb = use & 1;
+          const uint32_t bar = xbar + 8 * (warp * 2 + pb);
+          uint2* slot = xch + (size_t)(warp * 2 + pb) * CL * 32;
+          if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
+          const int zs = qd == 0 ? zq[0] : qd == 1 ? zq[1] : qd == 2 ? zq[2] : zq[3];
+          const float ls = qd == 0 ? lq[0] : qd == 1 ? lq[1] : qd == 2 ? lq[2] : lq[3];
+          const uint32_t la = smem_u32(slot + rank * 32 + lr + 8 * qd);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              const int row = wq * 32 + lr + 8 * k;
-              const uint32_t la = smem_u32(my_slot + (size_t)rank * kTileM + row);
-#pragma unroll
-              for (int p = 0; p < CL; ++p) st_cluster_f2(mapa(la, p), mloc[k], ls[k]);
-            }
-          }
-          __syncwarp();
-          if (lane == 0) {
-            asm volatile("fence.acq_rel.cluster;" ::: "memory");
-#pragma unroll
-            for (int p = 0; p < CL; ++p) mbar_arrive_remote(mapa(xbar + 8 * slot, p));
-          }
-          mbar_wait_cluster(xbar + 8 * slot, (use >> 1) & 1);
+          for (int p = 0; p < CL; ++p)
+            if (p != rank) st_async_b32x2(mapa(la, p), (uint32_t)zs, __float_as_uint(ls), mapa(bar, p));
+          mbar_wait(bar, (use >> 1) & 1);
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            const int row = wq * 32 + lr + 8 * k;
-            float M = -INFINITY;
-            float2 v[CL];
+            int Z = zq[k];
 #pragma unroll
-            for (int p = 0; p < CL; ++p) { v[p] = my_slot[(size_t)p * kTileM + row]; M = fmaxf(M, v[p].x); }
-            float l = 0.f;
+            for (int p = 0; p < CL; ++p)
+              if (p != rank) Z = max(Z, (int)slot[p * 32 + lr + 8 * k].x);
+            float L = 0.f;
 #pragma unroll
-            for (int p = 0; p < CL; ++p) l += (v[p].x == -INFINITY) ? 0.f : v[p].y * ex2(v[p].x - M);
-            w[k] = (mloc[k] == -INFINITY || !(l > 0.f)) ? 0.f : ex2(mloc[k] - M) / l;
+            for (int p = 0; p < CL; ++p) {   // rank order on every CTA: identical L bits cluster-wide
+              const uint2 v = slot[p * 32 + lr + 8 * k];
+              L += (p == rank) ? lq[k] * pow2i(zq[k] - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
+            }
+            zf[k] = Z; inv[k] = L > 0.f ? 1.f / L : 0.f;
           }
         }
+        // rows past the window contribute nothing
+        const int tok0 = c.q_row_begin + (tile % tok_tiles) * kTileM + wq * 32 + lr;
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (tok0 + wq * 32 + lr + 8 * k >= c.W) w[k] = 0.f;       // rows past the window contribute nothing
+        for (int k = 0; k < 4; ++k) if (tok0 + 8 * k >= c.W) inv[k] = 0.f;
+        float w[4][4];
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+#pragma unroll
+          for (int h2 = 0; h2 < 2; ++h2) {
+            const int za = (int)__byte_perm(zp[ch][h2], 0, 0x9910), zb = (int)__byte_perm(zp[ch][h2], 0, 0xBB32);
+            w[ch][2 * h2] = inv[2 * h2] * pow2i(za - zf[2 * h2]);
+            w[ch][2 * h2 + 1] = inv[2 * h2 + 1] * pow2i(zb - zf[2 * h2 + 1]);
+          }
+        }
 
         // ---- pass C: acc_j += sum_i e_ij w_i ----
-        for (int ch = 0; ch < n_chunks; ++ch) {
-          load_chunk(ch);
-          switch (ch) {   // compile-time accumulator indices
-#define KARA_ACC_CHUNK(CH)                                                                             \
-            case CH:                                                                                   \
-              _Pragma("unroll") for (int i = 0; i < 8; ++i) {                                          \
-                _Pragma("unroll") for (int j = 0; j < 2; ++j) {                                        \
-                  float a = acc[CH * 16 + 2 * i + j];                                                  \
-                  a = fmaf(__uint_as_float(r[4 * i + j]), w[0], a);                                    \
-                  a = fmaf(__uint_as_float(r[4 * i + 2 + j]), w[1], a);                                \
-                  a = fmaf(__uint_as_float(r[32 + 4 * i + j]), w[2], a);                               \
-                  a = fmaf(__uint_as_float(r[32 + 4 * i + 2 + j]), w[3], a);                           \
-                  acc[CH * 16 + 2 * i + j] = a;                                                        \
-                }                                                                                      \
-              }                                                                                        \
-              break;
-            KARA_ACC_CHUNK(0) KARA_ACC_CHUNK(1) KARA_ACC_CHUNK(2) KARA_ACC_CHUNK(3)
-#undef KARA_ACC_CHUNK
-          }
+        tmem_wait_st();
+        tmem_ld_16x256b_x8(taddr, ra);
+#define KARA_PASS_C(CH)                                                                        \
+        if (CH < n_chunks) {                                                                   \
+          tmem_wait_ld();                                                                      \
+          tmem_ld_16x256b_x8(taddr_hi + CH * 64, rb);                                          \
+          pass_c_half<CH, 0>(ra, acc, w);                                                      \
+          tmem_wait_ld();                                                                      \
+          if (CH + 1 < n_chunks) tmem_ld_16x256b_x8(taddr + (CH + 1) * 64, ra);                \
+          pass_c_half<CH, 2>(rb, acc, w);                                                      \
         }
-        // ---- release the TMEM buffer to the MMA warp ----
+        KARA_PASS_C(0) KARA_PASS_C(1) KARA_PASS_C(2) KARA_PASS_C(3)
+#undef KARA_PASS_C
+        // ---- release the TMEM buffer to the MMA warp (all of this warp's reads have completed) ----
         tc_fence_before();
-        named_bar_sync(1 + wg, 128);
-        if ((threadIdx.x & 127) == 0) mbar_arrive(tempty + 8 * buf);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty + 8 * wg);
       }
 
-      // ---- item done: combine lanes (fixed order), then warps (fixed order), write the strip ----
+      // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
 #pragma unroll
-      for (int a = 0; a < 64; ++a) {
-        float v = acc[a];
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        v += __shfl_xor_sync(0xffffffffu, v, 8);
-        v += __shfl_xor_sync(0xffffffffu, v, 16);
-        if (lr == 0) colsum[warp * kKeysPerCta + (a >> 4) * 64 + ((a & 15) >> 1) * 8 + 2 * qd + (a & 1)] = v;
-        acc[a] = 0.f;
+      for (int a = 0; a < 32; ++a) {
+        float v0, v1;
+        upk2(acc[a], v0, v1);
+        v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
+        v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
+        v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
+        if (lr == 0)
+          *reinterpret_cast<float2*>(&colsum[warp * kKeysPerCta + (a >> 3) * 64 + (a & 7) * 8 + 2 * qd]) =
+              make_float2(v0, v1);
+        acc[a] = 0ull;
       }
-      named_bar_sync(3, 32 * kSoftmaxWarps);
-      {
-        const int x = threadIdx.x;   // 0..255: one column each
+      named_bar_sync(1 + wg, 128);
+#pragma unroll
+      for (int x = threadIdx.x & 127; x < kKeysPerCta; x += 128) {
         float v = 0.f;
 #pragma unroll
-        for (int wv = 0; wv < kSoftmaxWarps; ++wv) v += colsum[wv * kKeysPerCta + x];
+        for (int wv = 0; wv < 4; ++wv) v += colsum[(wg * 4 + wv) * kKeysPerCta + x];
         if (x >= it.c_lo && x < it.c_hi) out[rank * kKeysPerCta + x - it.off] = v;
       }
-      named_bar_sync(3, 32 * kSoftmaxWarps);
+      named_bar_sync(1 + wg, 128);
     }
   }
 
@@ -606,8 +698,10 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
     attr_done = true;
   }
   const int tok_tiles = (c.W - c.q_row_begin + kTileM - 1) / kTileM;
-  const int tiles_per_unit = tok_tiles * c.G;
+  const int tpu = tok_tiles * c.G;
   const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;
+  const long long T = (long long)units * tpu;
+  if (T >= (1ll << 31)) return tc_fail(KARA_EUNSUPPORTED, "more than 2^31 query tiles in one call");
 
   cudaLaunchConfig_t cfg{};
   cudaLaunchAttribute attr[1];
@@ -623,26 +717,20 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
     cudaGetLastError();
     max_clusters = s->num_sms / CL;
   }
-  // split units into parts when that fills the last wave better (tail effect)
-  int best_parts = 1;
-  double best_eff = -1.0;
-  for (int parts = 1; parts <= 4 && parts <= tiles_per_unit; parts *= 2) {
-    const double items = (double)units * parts;
-    const double rounds = items / max_clusters;
-    const double eff = rounds / (double)((long long)((items + max_clusters - 1) / max_clusters)) - 0.015 * (parts - 1);
-    if (eff > best_eff + 1e-9) { best_eff = eff; best_parts = parts; }
-  }
-  c.parts = best_parts;
-  const int tiles_per_part = (tiles_per_unit + c.parts - 1) / c.parts;
-  const long long n_items = (long long)units * c.parts;
-  const int n_clusters = (int)(n_items < max_clusters ? n_items : max_clusters);
+  if (max_clusters > kMaxSms) max_clusters = kMaxSms;
+  const int n_clusters = (int)(T < max_clusters ? T : max_clusters);
   cfg.gridDim = dim3(CL * n_clusters);
+  c.part_T = (int)T; c.part_nc = n_clusters; c.part_tpu = tpu;
+  // every unit's strips must fit the workspace stride (strips_bound is the proof; this is the check)
+  const long long per_range = T / n_clusters;
+  long long ranges = (tpu - 1 + per_range - 1) / per_range + 1;
+  if (ranges > tpu) ranges = tpu;
+  if (2 * ranges > c.parts) return tc_fail(KARA_ENOMEM, "workspace holds too few partial-score strips per unit");
 
   CUtensorMap kmap, qmap;
   memcpy(&kmap, s->k_map, sizeof kmap);
   memcpy(&qmap, s->q_map, sizeof qmap);
-  cudaError_t e = cudaLaunchKernelEx(&cfg, kern, kmap, qmap, (const Call)c, (int)n_items, tiles_per_unit,
-                                     tiles_per_part, tok_tiles);
+  cudaError_t e = cudaLaunchKernelEx(&cfg, kern, kmap, qmap, (const Call)c, (int)T, tpu, tok_tiles);
   if (e != cudaSuccess) return tc_fail(KARA_ECUDA, cudaGetErrorString(e));
   return KARA_OK;
 }

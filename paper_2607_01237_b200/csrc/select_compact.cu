@@ -175,9 +175,10 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
 
   // ---- scores: sum the score kernel's partial column sums in part order -------------------
   const float* part = c.partial + (long long)unit * c.parts * n_pad;
+  const int n_strips = strips_of_unit(unit, c.parts, c.part_T, c.part_nc, c.part_tpu);
   for (int j = tid; j < n_pad; j += kThreads) {
     float a = 0.f;
-    if (j < n) for (int p = 0; p < c.parts; ++p) a += part[(long long)p * n_pad + j];
+    if (j < n) for (int p = 0; p < n_strips; ++p) a += part[(long long)p * n_pad + j];
     s_A[j] = a;
     s_key[j] = key_of(a);
     s_sel[j] = 0;
