@@ -20,7 +20,8 @@ OBJ = HERE / "build"
 SO = HERE / "libkara.so"
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-         "-Xcompiler", "-fPIC,-Wall,-Wextra", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
+         "-Xcompiler", "-fPIC,-Wall,-Wextra", "-Xptxas", "-v", "--expt-relaxed-constexpr",
+         *os.environ.get("KARA_NVCC_EXTRA", "").split()]   # e.g. -DKARA_TC_DEBUG (mbarrier watchdog)
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:

@@ -1,4 +1,4 @@
-// score_tc.cu — a1 (Eq. 4): A = colsum(softmax(Q_W K_{W\U}^T / sqrt(d))) on the
+// score_tc.cu — a1 (Eq. 4): A = colsum(softmax(Q_W K_{W\\U}^T / sqrt(d))) on the
 // 5th-generation tensor cores of sm_100a: TMA -> shared memory, tcgen05.mma -> TMEM, softmax out
 // of TMEM, deterministic column sums.  DESIGN.md §Kernels/a1 has the derivation of every choice.
 //
@@ -11,24 +11,29 @@
 // 256 key rows [256 r, 256 r + 256) of the block-aligned key panel (whole paged blocks are
 // loaded, one TMA box per block and 64-element column panel; rows outside the compressible
 // region [h, h+n) are masked to -inf).  Per tile and CTA:
-//   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM
+//   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM,
+//       issued as two N <= 128 halves with their own full / empty barriers.
+//   Four softmax warpgroups: WG (b, hf) works on TMEM buffer b (tiles alternate between the two
+//       buffers) and on column half hf of it, so four warps share every SM sub-partition and the
+//       MUFU pipe always has a warp with work (the v2 kernel had two and was latency bound).
 //   pass B (one TMEM read, one write):  a thread holds 4 rows x 16 columns of a 64-column chunk;
 //       it shifts by ITS OWN maximum of those 16 logits, rounded to an integer z (log2 domain):
 //       e = exp2(s c - z), written back in place; l += e.  No separate max pass, no shuffles.
-//   statistics: z and l of the (<= 4) chunks, the 4 lanes of a row and the CL CTAs of the
-//       cluster are merged with exact power-of-two rescaling built by integer arithmetic (no
-//       MUFU); across CTAs through distributed shared memory with st.async + a transaction-count
-//       mbarrier per warp (no fence, no cluster barrier).  w_(row,chunk) = 2^(z - Z_row) / L_row.
+//   statistics: (z, l) of a row are merged over the thread's chunks, the 4 lanes of the row, the
+//       two column halves and the CL CTAs with exact power-of-two rescaling built by integer
+//       arithmetic (no MUFU).  Every (CTA, half) publishes its 128 rows to every CTA of the
+//       cluster (its own included) with st.async + a transaction-count mbarrier per (buffer, warp
+//       quadrant) — no fence, no cluster barrier.  w_(row,chunk) = 2^(z - Z_row) / L_row.
 //   pass C (one TMEM read):  acc_j += sum_i e_ij w_i   per-thread registers: with the 16x256b
 //       TMEM load shape the column sum over ALL tiles of a segment is a plain packed FFMA2;
 //       lanes are combined once per segment.
-// TMEM holds two 128 x 256 fp32 S buffers (all 512 columns): the MMA of the next tile of a
-// warpgroup runs while the other warpgroup is in its softmax; two softmax warpgroups alternate
-// tiles.  The K panel is double-buffered so a segment change costs no bubble.
+// TMEM holds two 128 x 256 fp32 S buffers (all 512 columns).  The K panel is double-buffered so a
+// segment change costs no bubble.
 //
-// Warp roles (384 threads): warps 0-3 softmax WG0, 4-7 softmax WG1, 8 TMA producer, 9 MMA issuer,
-// 10-11 idle (they exist so that setmaxnreg can move their registers to the softmax warpgroups).
-// Output: partial[unit][2 p + wg][j] (fp32), p = index of the range among those that touch the
+// Warp roles (640 threads): warps 0-15 softmax (WG g = warp/4 = 2 b + hf, 112 registers), 16 TMA
+// producer, 17 MMA issuer, 18-19 idle (32 registers; they complete the warpgroup whose registers
+// setmaxnreg hands to the softmax warps).
+// Output: partial[unit][2 p + b][j] (fp32), p = index of the range among those that touch the
 // unit; the select kernel sums the strips in fixed order, so scores are bit-reproducible run to
 // run (no atomics anywhere).
 #include <cuda.h>
@@ -42,20 +47,26 @@ namespace kara {
 
 namespace {
 
-constexpr int kSoftmaxWarps = 8;
-constexpr int kProducerWarp = 8;
-constexpr int kMmaWarp = 9;
-constexpr int kThreads = 32 * 12;             // 3 warpgroups (setmaxnreg works per warpgroup); warps 10, 11 idle
-constexpr int kRegsSoftmax = 232, kRegsOther = 40;   // 168 x 384 at launch -> 2 x 128 x 232 + 128 x 40
+constexpr int kSoftmaxWarps = 16;
+constexpr int kProducerWarp = 16;
+constexpr int kMmaWarp = 17;
+constexpr int kThreads = 32 * 20;             // 5 warpgroups (setmaxnreg works per warpgroup); warps 18, 19 idle
+// setmaxnreg only moves registers inside the CTA's launch allocation (640 x 96; registers are
+// allocated per 4 warps, so 18 warps cost as much as 20): 512 x (112 - 96) <= 128 x (96 - 32)
+constexpr int kRegsSoftmax = 112, kRegsOther = 32;
 constexpr int kTileM = 128;
 constexpr int kKeysPerCta = 256;
+constexpr int kHalf = 128;                    // columns of one softmax warpgroup / of one MMA
 constexpr int kQStages = 2;
 constexpr int kTmemCols = 512;
-constexpr float kZLim = 32000.f;              // integer shifts z are clamped to +-kZLim (|logit| log2e / sqrt(d) beyond that is not served)
-constexpr uint32_t kZEmptyPair = 0x83008300u; // two int16 -32000: the shift of a piece with no valid key
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kMagic = 12582912.f;          // 1.5 * 2^23: x + kMagic rounds x to an integer in the low mantissa bits
 constexpr int kMagicBits = 0x4B400000;
+// integer shifts z are carried as the bit pattern of (z + kMagic), i.e. biased by kMagicBits; they
+// are clamped to z <= kZLim (|logit| log2e / sqrt(d) beyond that is not served) and floored at
+// -kZLim, which is also the shift of a piece with no valid key (its l is 0)
+constexpr float kZLim = 32000.f;
+constexpr int kZFloor = kMagicBits - 32000;
 
 char g_tc_err[256] = "";
 
@@ -76,6 +87,22 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
 }
+#ifdef KARA_TC_DEBUG
+// debug build: a wait that does not complete within ~2^26 polls reports who is stuck and traps
+__device__ __noinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  for (long long spin = 0;; ++spin) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+    if (spin > (1ll << 24)) {
+      printf("STUCK block %d warp %d lane %d bar_off %u parity %u\n", blockIdx.x, threadIdx.x >> 5, threadIdx.x & 31,
+             bar & 1023u, parity);
+      __trap();
+    }
+  }
+}
+#else
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
@@ -86,6 +113,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "KARA_DONE_%=:\n\t}"
       :: "r"(bar), "r"(parity) : "memory");
 }
+#endif
 __device__ __forceinline__ uint32_t mapa(uint32_t local_addr, uint32_t cta) {
   uint32_t r;
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta));
@@ -222,16 +250,17 @@ __device__ __forceinline__ float pow2i(int d) { return __int_as_float(max(d + 12
 template <int D, int CL>
 struct Smem {
   static constexpr int kPanels = D / 64;
-  static constexpr int kKStages = CL >= 8 ? 1 : 2;   // 8-CTA clusters need the room for the exchange slots
+  static constexpr int kKStages = CL >= 4 ? 1 : 2;   // larger clusters need the room for the exchange slots
   static constexpr int kKBytes = kPanels * kKeysPerCta * 128;
   static constexpr int kQStageBytes = kPanels * kTileM * 128;
+  static constexpr int kParticipants = 2 * CL;       // (CTA, column half) pairs that own a piece of a row
   static constexpr int kOffK = 0;
   static constexpr int kOffQ = kOffK + kKStages * kKBytes;
-  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;            // float [8][256]
-  static constexpr int kOffXch = kOffColsum + kSoftmaxWarps * kKeysPerCta * 4;  // uint2 [8 warps][2][CL][32]
-  static constexpr int kOffBars = kOffXch + kSoftmaxWarps * 2 * CL * 32 * 8;
-  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2] tempty[2] xbar[8][2]  = 28 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 28 * 8;
+  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;            // float [16 warps][128]
+  static constexpr int kOffXch = kOffColsum + kSoftmaxWarps * kHalf * 4;        // uint2 [8 groups][2][2 CL][32]
+  static constexpr int kOffBars = kOffXch + 8 * 2 * kParticipants * 32 * 8;
+  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] xbar[8][2]  = 32 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 32 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
@@ -241,7 +270,7 @@ struct Seg {
   int unit, part, li, s, hk, layer;
   int h, fb, off;          // window start, first key block (table index), h - fb*bs
   int c_lo, c_hi;          // this CTA's valid key columns [c_lo, c_hi) within its 256
-  int n_cols;              // MMA N for this CTA: valid columns rounded up to 16 (>= 16)
+  int n_cols;              // columns the MMAs of this CTA produce: valid columns rounded up to 16 (>= 16)
   int t0, t1;
   bool ok;
 };
@@ -271,16 +300,18 @@ __device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long 
   it.n_cols = max(16, (it.c_hi + 15) & ~15);
   return it;
 }
+// columns of half hf that the MMA produces (0 = the half is not computed at all)
+__device__ __forceinline__ int half_cols(const Seg& it, int hf) { return min(max(it.n_cols - hf * kHalf, 0), kHalf); }
 
-// ---- pass B on one half-chunk: 2 rows (K0, K0+1) x 16 columns of chunk C held in r[32] ----------
-// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column 64 C + 8 i + 2 qd + j.
+// ---- pass B on one piece: 2 rows (K0, K0+1) x 16 columns of chunk C (of this half) held in r[32] ----
+// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column 64 C + 8 i + 2 qd + j (relative to the half).
 // Online softmax with exact power-of-two rescaling: the shift of this (row, chunk) is the running
 // maximum z = max(z_run, round(m c)) of the thread's integer shifts (log2 domain), so e <= 2^0.5;
-// l_run is rescaled by 2^(z_old - z) built from the exponent field (no MUFU).  z is clamped to
-// [-kZLim, kZLim] and kept as int16 (zp); a fully masked piece has m = -inf -> z = -kZLim, e = 0.
+// l_run is rescaled by 2^(z_old - z) built from the exponent field (no MUFU).  Shifts are biased
+// ints (see kZFloor); a fully masked piece has m = -inf -> as_int(t) < 0 -> z = floor / z_run, e = 0.
 template <int C, int K0>
-__device__ __forceinline__ void pass_b_half(uint32_t (&r)[32], uint32_t (&zp)[4][2], int (&zrun)[4], float (&lrun)[4],
-                                            float cs, int qd, int c_lo, int c_hi) {
+__device__ __forceinline__ void pass_b_piece(uint32_t (&r)[32], int (&zc)[2][4], int (&zrun)[4], float (&lrun)[4],
+                                             float cs, int qd, int c_lo, int c_hi) {
   constexpr int cb = C * 64;
   if (!(cb >= c_lo && cb + 64 <= c_hi)) {   // warp-uniform: only the ragged first / last chunk
 #pragma unroll
@@ -302,14 +333,16 @@ __device__ __forceinline__ void pass_b_half(uint32_t (&r)[32], uint32_t (&zp)[4]
   m0 = max3(m0, KARA_F(28), KARA_F(29));   m1 = max3(m1, KARA_F(30), KARA_F(31));
   m0 = fmaxf(m0, m0b);                     m1 = fmaxf(m1, m1b);
 #undef KARA_F
-  const float t0 = fminf(fmaxf(m0 * cs, -kZLim), kZLim) + kMagic;   // integer in the low mantissa bits
-  const float t1 = fminf(fmaxf(m1 * cs, -kZLim), kZLim) + kMagic;
-  const int z0 = max(zrun[K0], __float_as_int(t0) - kMagicBits);
-  const int z1 = max(zrun[K0 + 1], __float_as_int(t1) - kMagicBits);
-  const float l0s = lrun[K0] * pow2i(zrun[K0] - z0), l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
+  // t = round(m c) + kMagic as a float; its bit pattern is the biased integer shift
+  const float t0 = fminf(fmaf(m0, cs, kMagic), kMagic + kZLim);
+  const float t1 = fminf(fmaf(m1, cs, kMagic), kMagic + kZLim);
+  const int z0 = max(zrun[K0], __float_as_int(t0)), z1 = max(zrun[K0 + 1], __float_as_int(t1));
+  float l0s, l1s;
+  if (C == 0) { l0s = 0.f; l1s = 0.f; }     // first chunk of the tile: nothing accumulated yet
+  else { l0s = lrun[K0] * pow2i(zrun[K0] - z0); l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1); }
   zrun[K0] = z0; zrun[K0 + 1] = z1;
-  zp[C][K0 / 2] = ((uint32_t)z0 & 0xffffu) | ((uint32_t)z1 << 16);
-  const float nz0 = kMagic - __int_as_float(z0 + kMagicBits), nz1 = kMagic - __int_as_float(z1 + kMagicBits);
+  zc[C][K0] = z0; zc[C][K0 + 1] = z1;
+  const float nz0 = kMagic - __int_as_float(z0), nz1 = kMagic - __int_as_float(z1);   // = -z, exact
   const uint64_t cs2 = pk2(cs, cs), nz0_2 = pk2(nz0, nz0), nz1_2 = pk2(nz1, nz1);
   uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
 #pragma unroll
@@ -329,9 +362,9 @@ __device__ __forceinline__ void pass_b_half(uint32_t (&r)[32], uint32_t (&zp)[4]
   upk2(l1, a, b); lrun[K0 + 1] = a + b;
 }
 
-// ---- pass C on one half-chunk: acc[C*8 + i] (columns 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------
+// ---- pass C on one piece: acc[C*8 + i] (columns 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------------
 template <int C, int K0>
-__device__ __forceinline__ void pass_c_half(const uint32_t (&r)[32], uint64_t (&acc)[32], const float (&w)[4][4]) {
+__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[16], const float (&w)[2][4]) {
   const uint64_t w0 = pk2(w[C][K0], w[C][K0]), w1 = pk2(w[C][K0 + 1], w[C][K0 + 1]);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
@@ -360,7 +393,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
   const uint32_t qfull = bars, qempty = bars + 16, kfull = bars + 32, kempty = bars + 48;
-  const uint32_t tfull = bars + 64, tempty = bars + 80, xbar = bars + 96;
+  const uint32_t tfull = bars + 64, tempty = bars + 96, xbar = bars + 128;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -373,16 +406,18 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     for (int i = 0; i < 2; ++i) {
       mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1);
       mbar_init(kfull + 8 * i, 1); mbar_init(kempty + 8 * i, 1);
+    }
+    for (int i = 0; i < 4; ++i) {
       mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 4);   // one arrive per warp of the warpgroup
     }
-    for (int i = 0; i < 16; ++i) mbar_init(xbar + 8 * i, 1);       // per softmax warp and parity
+    for (int i = 0; i < 16; ++i) mbar_init(xbar + 8 * i, 2);       // per (buffer, warp quadrant) and parity: the two halves' warps arrive
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  if (CL > 1) cluster_sync_all();
+  cluster_sync_all();
   const uint32_t tmem_base = *tmem_ptr;
 
   if (warp >= kSoftmaxWarps) {
@@ -457,96 +492,111 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     }
   } else if (warp == kMmaWarp) {
     // ================================ MMA issuer ================================================
-    int q_iter = 0, k_iter = 0, tile_iter = 0;
-    for (long long g = g_begin; g < g_end;) {
-      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
-      g += it.t1 - it.t0;
-      if (!it.ok) continue;
-      const uint32_t idesc = make_idesc_bf16(it.n_cols);
-      const int kstage = k_iter % SM::kKStages, kuse = k_iter / SM::kKStages;
-      ++k_iter;
-      if (lane == 0) {
+    if (lane == 0) {
+      int q_iter = 0, k_iter = 0, tile_iter = 0;
+      uint32_t t_par = 0;                      // bit (2 buf + hf): parity of the next use of that half buffer
+      for (long long g = g_begin; g < g_end;) {
+        const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+        g += it.t1 - it.t0;
+        if (!it.ok) continue;
+        const int nc0 = half_cols(it, 0), nc1 = half_cols(it, 1);
+        const int kstage = k_iter % SM::kKStages, kuse = k_iter / SM::kKStages;
+        ++k_iter;
         mbar_wait(kfull + 8 * kstage, kuse & 1);
         for (int tile = it.t0; tile < it.t1; ++tile, ++q_iter, ++tile_iter) {
           const int stage = q_iter % kQStages, quse = q_iter / kQStages;
-          const int buf = tile_iter & 1, tuse = tile_iter >> 1;
+          const int buf = tile_iter & 1;
           mbar_wait(qfull + 8 * stage, quse & 1);
-          mbar_wait(tempty + 8 * buf, (tuse & 1) ^ 1);
-          tc_fence_after();
-          const uint32_t d_tmem = tmem_base + buf * kKeysPerCta;
 #pragma unroll
-          for (int p = 0; p < SM::kPanels; ++p) {
+          for (int hf = 0; hf < 2; ++hf) {
+            const int nc = hf ? nc1 : nc0;
+            if (nc == 0) continue;
+            const int slot = 2 * buf + hf;
+            mbar_wait(tempty + 8 * slot, ((t_par >> slot) & 1) ^ 1);
+            t_par ^= 1u << slot;
+            tc_fence_after();
+            const uint32_t d_tmem = tmem_base + buf * kKeysPerCta + hf * kHalf;
+            const uint32_t idesc = make_idesc_bf16(nc);
 #pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {
-              const uint64_t ad = make_sw128_desc(sQ + stage * SM::kQStageBytes + p * (kTileM * 128) + ks * 32);
-              const uint64_t bd = make_sw128_desc(sK + kstage * SM::kKBytes + p * (kKeysPerCta * 128) + ks * 32);
-              umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
+            for (int p = 0; p < SM::kPanels; ++p) {
+#pragma unroll
+              for (int ks = 0; ks < 4; ++ks) {
+                const uint64_t ad = make_sw128_desc(sQ + stage * SM::kQStageBytes + p * (kTileM * 128) + ks * 32);
+                const uint64_t bd = make_sw128_desc(sK + kstage * SM::kKBytes + p * (kKeysPerCta * 128) +
+                                                    hf * (kHalf * 128) + ks * 32);
+                umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
+              }
             }
+            if (hf == 1 || nc1 == 0) umma_commit(qempty + 8 * stage);   // Q stage reusable once these MMAs have read it
+            umma_commit(tfull + 8 * slot);                               // this half of the S tile is complete
           }
-          umma_commit(qempty + 8 * stage);   // Q stage reusable once these MMAs have read it
-          umma_commit(tfull + 8 * buf);      // S tile complete
         }
         umma_commit(kempty + 8 * kstage);    // K stage reusable
-      } else {
-        const int nt = it.t1 - it.t0;
-        q_iter += nt; tile_iter += nt;
       }
-      __syncwarp();
     }
+    __syncwarp();
   }
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsSoftmax));
     // ================================ softmax warpgroups =========================================
+    constexpr int P = SM::kParticipants;
     const int wg = warp >> 2, wq = warp & 3;
+    const int b = wg >> 1, hf = wg & 1;                 // TMEM buffer, column half
     const int qd = lane & 3, lr = lane >> 2;            // column pair within a group of 8; row within 8
+    const int grp = b * 4 + wq;                         // exchange group: the warps that hold the same 32 rows
     const float cs = kLog2e * rsqrtf((float)D);
-    const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + wg * kKeysPerCta;
+    const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + b * kKeysPerCta + hf * kHalf;
     const uint32_t taddr_hi = taddr + (16u << 16);
-    uint64_t acc[32];
+    const uint32_t tf = tfull + 8 * (2 * b + hf), te = tempty + 8 * (2 * b + hf);
+    uint64_t acc[16];
 #pragma unroll
-    for (int a = 0; a < 32; ++a) acc[a] = 0ull;
-    int tile_iter = 0, my_use = 0;
+    for (int a = 0; a < 16; ++a) acc[a] = 0ull;
+    int tile_iter = 0, x_use = 0, t_use = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
-      float* out = c.partial + ((long long)it.unit * c.parts + 2 * it.part + wg) * c.n_pad;
+      float* out = c.partial + ((long long)it.unit * c.parts + 2 * it.part + b) * c.n_pad;
       if (!it.ok) {
         // skipped unit: its strips must still be defined (zeros); the status word says why
-        if (rank == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
+        if (rank == 0 && hf == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
         continue;
       }
-      const int n_chunks = (it.n_cols + 63) >> 6;
+      const int n_chunks = (half_cols(it, hf) + 63) >> 6;                       // 0, 1 or 2
+      const int h_lo = min(max(it.c_lo - hf * kHalf, 0), kHalf), h_hi = min(max(it.c_hi - hf * kHalf, 0), kHalf);
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        if ((tile_iter & 1) != wg) continue;
-        const int use = my_use++;
-        mbar_wait(tfull + 8 * wg, (tile_iter >> 1) & 1);
-        tc_fence_after();
-
-        // ---- pass B: e = 2^(s c - z) in place; z (int16 pairs) per (row, chunk), running (z, l) per row ----
-        uint32_t zp[4][2];
-        int zq[4];
+        if ((tile_iter & 1) != b) continue;
+        const int use = x_use++;
+        int zc[2][4], zq[4];
         float lq[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { zq[k] = -(int)kZLim; lq[k] = 0.f; }
-#pragma unroll
-        for (int ch = 0; ch < 4; ++ch) { zp[ch][0] = zp[ch][1] = kZEmptyPair; }
-        uint32_t ra[32], rb[32];
-        tmem_ld_16x256b_x8(taddr, ra);
-#define KARA_PASS_B(CH)                                                                        \
-        if (CH < n_chunks) {                                                                   \
-          tmem_wait_ld();                                                                      \
-          tmem_ld_16x256b_x8(taddr_hi + CH * 64, rb);                                          \
-          pass_b_half<CH, 0>(ra, zp, zq, lq, cs, qd, it.c_lo, it.c_hi);                        \
-          tmem_st_16x256b_x8(taddr + CH * 64, ra);                                             \
-          tmem_wait_ld();                                                                      \
-          if (CH + 1 < n_chunks) tmem_ld_16x256b_x8(taddr + (CH + 1) * 64, ra);                \
-          pass_b_half<CH, 2>(rb, zp, zq, lq, cs, qd, it.c_lo, it.c_hi);                        \
-          tmem_st_16x256b_x8(taddr_hi + CH * 64, rb);                                          \
+        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; }
+        uint32_t r[32];
+        if (n_chunks > 0) {
+          mbar_wait(tf, t_use & 1);
+          ++t_use;
+          tc_fence_after();
+          // ---- pass B: e = 2^(s c - z) in place; z per (row, chunk), running (z, l) per row ----
+          tmem_ld_16x256b_x8(taddr, r);
+          tmem_wait_ld();
+          pass_b_piece<0, 0>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
+          tmem_st_16x256b_x8(taddr, r);
+          tmem_ld_16x256b_x8(taddr_hi, r);
+          tmem_wait_ld();
+          pass_b_piece<0, 2>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
+          tmem_st_16x256b_x8(taddr_hi, r);
+          if (n_chunks > 1) {
+            tmem_ld_16x256b_x8(taddr + 64, r);
+            tmem_wait_ld();
+            pass_b_piece<1, 0>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
+            tmem_st_16x256b_x8(taddr + 64, r);
+            tmem_ld_16x256b_x8(taddr_hi + 64, r);
+            tmem_wait_ld();
+            pass_b_piece<1, 2>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
+            tmem_st_16x256b_x8(taddr_hi + 64, r);
+          }
         }
-        KARA_PASS_B(0) KARA_PASS_B(1) KARA_PASS_B(2) KARA_PASS_B(3)
-#undef KARA_PASS_B
 
-        // ---- row statistics: quad -> CTA, cluster -> row ----
+        // ---- row statistics: quad -> (CTA, half); then every (CTA, half) of the cluster -> row ----
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const int zt = zq[k];
@@ -557,103 +607,106 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           lt += __shfl_xor_sync(0xffffffffu, lt, 2);
           zq[k] = zz; lq[k] = lt;
         }
-        int zf[4];
-        float inv[4];
-        if (CL == 1) {
-#pragma unroll
-          for (int k = 0; k < 4; ++k) { zf[k] = zq[k]; inv[k] = lq[k] > 0.f ? 1.f / lq[k] : 0.f; }
-        } else {
-          // lane (lr, qd) publishes row lr + 8 qd of this warp to every peer CTA
+        float inv_row;
+        int z_row;
+        {
+          // lane (lr, qd) publishes row lr + 8 qd of this warp to every CTA (its own included) ...
           const int pb = use & 1;
-          const uint32_t bar = xbar + 8 * (warp * 2 + pb);
-          uint2* slot = xch + (size_t)(warp * 2 + pb) * CL * 32;
-          if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
+          const uint32_t bar = xbar + 8 * (grp * 2 + pb);
+          uint2* slot = xch + (size_t)(grp * 2 + pb) * P * 32;
           const int zs = qd == 0 ? zq[0] : qd == 1 ? zq[1] : qd == 2 ? zq[2] : zq[3];
           const float ls = qd == 0 ? lq[0] : qd == 1 ? lq[1] : qd == 2 ? lq[2] : lq[3];
-          const uint32_t la = smem_u32(slot + rank * 32 + lr + 8 * qd);
-#pragma unroll
-          for (int p = 0; p < CL; ++p)
-            if (p != rank) st_async_b32x2(mapa(la, p), (uint32_t)zs, __float_as_uint(ls), mapa(bar, p));
-          mbar_wait(bar, (use >> 1) & 1);
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            int Z = zq[k];
+          const int row = lr + 8 * qd;
+          uint2* mine = slot + (rank * 2 + hf) * 32 + row;
+          *mine = make_uint2((uint32_t)zs, __float_as_uint(ls));              // own CTA: plain store + arrive
+          if (CL > 1) {
+            const uint32_t la = smem_u32(mine);
 #pragma unroll
             for (int p = 0; p < CL; ++p)
-              if (p != rank) Z = max(Z, (int)slot[p * 32 + lr + 8 * k].x);
-            float L = 0.f;
-#pragma unroll
-            for (int p = 0; p < CL; ++p) {   // rank order on every CTA: identical L bits cluster-wide
-              const uint2 v = slot[p * 32 + lr + 8 * k];
-              L += (p == rank) ? lq[k] * pow2i(zq[k] - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
-            }
-            zf[k] = Z; inv[k] = L > 0.f ? 1.f / L : 0.f;
+              if (p != rank) st_async_b32x2(mapa(la, p), (uint32_t)zs, __float_as_uint(ls), mapa(bar, p));
           }
-        }
-        // rows past the window contribute nothing
-        const int tok0 = c.q_row_begin + (tile % tok_tiles) * kTileM + wq * 32 + lr;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) if (tok0 + 8 * k >= c.W) inv[k] = 0.f;
-        float w[4][4];
-#pragma unroll
-        for (int ch = 0; ch < 4; ++ch) {
-#pragma unroll
-          for (int h2 = 0; h2 < 2; ++h2) {
-            const int za = (int)__byte_perm(zp[ch][h2], 0, 0x9910), zb = (int)__byte_perm(zp[ch][h2], 0, 0xBB32);
-            w[ch][2 * h2] = inv[2 * h2] * pow2i(za - zf[2 * h2]);
-            w[ch][2 * h2 + 1] = inv[2 * h2 + 1] * pow2i(zb - zf[2 * h2 + 1]);
+          __syncwarp();
+          if (lane == 0) {
+            if (CL > 1 && hf == 0) mbar_expect_tx(bar, (P - 2) * 32 * 8);    // the peers' bytes; counts as this warp's arrive
+            else mbar_arrive(bar);
           }
+          mbar_wait(bar, (use >> 1) & 1);
+          // ... and merges that row over all participants (participant order: identical bits everywhere)
+          uint2 v[P];
+#pragma unroll
+          for (int p = 0; p < P; ++p) v[p] = slot[p * 32 + row];
+          int Z = (int)v[0].x;
+#pragma unroll
+          for (int p = 1; p < P; ++p) Z = max(Z, (int)v[p].x);
+          float L = 0.f;
+#pragma unroll
+          for (int p = 0; p < P; ++p) L += __uint_as_float(v[p].y) * pow2i((int)v[p].x - Z);
+          const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + wq * 32 + row;
+          inv_row = (L > 0.f && tok < c.W) ? 1.f / L : 0.f;     // rows past the window contribute nothing
+          z_row = Z;
         }
-
-        // ---- pass C: acc_j += sum_i e_ij w_i ----
-        tmem_wait_st();
-        tmem_ld_16x256b_x8(taddr, ra);
-#define KARA_PASS_C(CH)                                                                        \
-        if (CH < n_chunks) {                                                                   \
-          tmem_wait_ld();                                                                      \
-          tmem_ld_16x256b_x8(taddr_hi + CH * 64, rb);                                          \
-          pass_c_half<CH, 0>(ra, acc, w);                                                      \
-          tmem_wait_ld();                                                                      \
-          if (CH + 1 < n_chunks) tmem_ld_16x256b_x8(taddr + (CH + 1) * 64, ra);                \
-          pass_c_half<CH, 2>(rb, acc, w);                                                      \
+        if (n_chunks > 0) {
+          float w[2][4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const int zf = __shfl_sync(0xffffffffu, z_row, (lr << 2) | k);
+            const float iv = __shfl_sync(0xffffffffu, inv_row, (lr << 2) | k);
+            w[0][k] = iv * pow2i(zc[0][k] - zf);
+            w[1][k] = n_chunks > 1 ? iv * pow2i(zc[1][k] - zf) : 0.f;
+          }
+          // ---- pass C: acc_j += sum_i e_ij w_i ----
+          tmem_wait_st();
+          tmem_ld_16x256b_x8(taddr, r);
+          tmem_wait_ld();
+          pass_c_piece<0, 0>(r, acc, w);
+          tmem_ld_16x256b_x8(taddr_hi, r);
+          tmem_wait_ld();
+          pass_c_piece<0, 2>(r, acc, w);
+          if (n_chunks > 1) {
+            tmem_ld_16x256b_x8(taddr + 64, r);
+            tmem_wait_ld();
+            pass_c_piece<1, 0>(r, acc, w);
+            tmem_ld_16x256b_x8(taddr_hi + 64, r);
+            tmem_wait_ld();
+            pass_c_piece<1, 2>(r, acc, w);
+          }
+          // ---- release this half of the TMEM buffer to the MMA warp (all of this warp's reads have completed) ----
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(te);
         }
-        KARA_PASS_C(0) KARA_PASS_C(1) KARA_PASS_C(2) KARA_PASS_C(3)
-#undef KARA_PASS_C
-        // ---- release the TMEM buffer to the MMA warp (all of this warp's reads have completed) ----
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tempty + 8 * wg);
       }
 
       // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
+      if (n_chunks > 0) {
 #pragma unroll
-      for (int a = 0; a < 32; ++a) {
-        float v0, v1;
-        upk2(acc[a], v0, v1);
-        v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
-        v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
-        v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
-        if (lr == 0)
-          *reinterpret_cast<float2*>(&colsum[warp * kKeysPerCta + (a >> 3) * 64 + (a & 7) * 8 + 2 * qd]) =
-              make_float2(v0, v1);
-        acc[a] = 0ull;
+        for (int a = 0; a < 16; ++a) {
+          float v0, v1;
+          upk2(acc[a], v0, v1);
+          v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
+          v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
+          v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
+          if (lr == 0)
+            *reinterpret_cast<float2*>(&colsum[warp * kHalf + (a >> 3) * 64 + (a & 7) * 8 + 2 * qd]) = make_float2(v0, v1);
+          acc[a] = 0ull;
+        }
+        named_bar_sync(1 + wg, 128);
+        {
+          const int x = threadIdx.x & 127;
+          float v = 0.f;
+#pragma unroll
+          for (int wv = 0; wv < 4; ++wv) v += colsum[(wg * 4 + wv) * kHalf + x];
+          if (x >= h_lo && x < h_hi) out[rank * kKeysPerCta + hf * kHalf + x - it.off] = v;
+        }
+        named_bar_sync(1 + wg, 128);
       }
-      named_bar_sync(1 + wg, 128);
-#pragma unroll
-      for (int x = threadIdx.x & 127; x < kKeysPerCta; x += 128) {
-        float v = 0.f;
-#pragma unroll
-        for (int wv = 0; wv < 4; ++wv) v += colsum[(wg * 4 + wv) * kKeysPerCta + x];
-        if (x >= it.c_lo && x < it.c_hi) out[rank * kKeysPerCta + x - it.off] = v;
-      }
-      named_bar_sync(1 + wg, 128);
     }
   }
 
   // ---- teardown: nobody may exit while a peer can still write into this CTA ----
   tc_fence_before();
   __syncthreads();
-  if (CL > 1) cluster_sync_all();
+  cluster_sync_all();
   if (warp == kMmaWarp) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
 }
 
