@@ -39,7 +39,7 @@ struct Call {
   // Which strips of a unit hold data.  part_T == 0: all `parts` strips (SIMT kernel).  part_T > 0
   // (tcgen05 kernel): the T = units*part_tpu query tiles are split into part_nc contiguous ranges,
   // one per cluster; a unit's tiles touch clusters [tile_owner(first), tile_owner(last)] and each
-  // of them writes two strips (one per softmax warpgroup): strips_of_unit().
+  // of them writes kScoreStrips strips: strips_of_unit().
   int part_T, part_nc, part_tpu;
   int keep_debug;
   int32_t* free_list;
@@ -51,6 +51,7 @@ struct WsLayout {
   int parts, n_pad, k_pad, keep_pad;
 };
 
+constexpr int kScoreStrips = 1; // strips a range writes per unit
 constexpr int kMaxSms = 160;    // upper bound on clusters of one launch (B200: 148 SMs)
 constexpr int kMaxN = 2048;     // largest compressible region (cfg 5: 1984)
 
@@ -65,7 +66,7 @@ __host__ __device__ inline int tile_owner(long long tile, int nc, int T) {
 __host__ __device__ inline int strips_of_unit(int unit, int parts, int part_T, int part_nc, int part_tpu) {
   if (part_T <= 0) return parts;
   const long long first = (long long)unit * part_tpu;
-  return 2 * (tile_owner(first + part_tpu - 1, part_nc, part_T) - tile_owner(first, part_nc, part_T) + 1);
+  return kScoreStrips * (tile_owner(first + part_tpu - 1, part_nc, part_T) - tile_owner(first, part_nc, part_T) + 1);
 }
 // Upper bound of strips_of_unit over every split of units*tpu tiles into <= kMaxSms ranges: a
 // range holds >= p = floor(T/nc) tiles, so the tpu consecutive tiles of a unit meet at most
@@ -75,7 +76,7 @@ inline int strips_bound(int units, int tpu) {
   if (p < 1) p = 1;
   long long ranges = (tpu - 1 + p - 1) / p + 1;
   if (ranges > tpu) ranges = tpu;
-  return (int)(2 * ranges);
+  return (int)(kScoreStrips * ranges);
 }
 
 // unit index -> (layer-in-call, sequence, kv head)

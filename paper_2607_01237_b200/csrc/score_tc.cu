@@ -12,30 +12,32 @@
 // loaded, one TMA box per block and 64-element column panel; rows outside the compressible
 // region [h, h+n) are masked to -inf).  Per tile and CTA:
 //   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM,
-//       issued as two N <= 128 halves with their own full / empty barriers.
-//   Four softmax warpgroups: WG (b, hf) works on TMEM buffer b (tiles alternate between the two
-//       buffers) and on column half hf of it, so four warps share every SM sub-partition and the
-//       MUFU pipe always has a warp with work (the v2 kernel had two and was latency bound).
-//   pass B (one TMEM read, one write):  a thread holds 4 rows x 16 columns of a 64-column chunk;
-//       it shifts by ITS OWN maximum of those 16 logits, rounded to an integer z (log2 domain):
-//       e = exp2(s c - z), written back in place; l += e.  No separate max pass, no shuffles.
-//   statistics: (z, l) of a row are merged over the thread's chunks, the 4 lanes of the row, the
-//       two column halves and the CL CTAs with exact power-of-two rescaling built by integer
-//       arithmetic (no MUFU).  Every (CTA, half) publishes its 128 rows to every CTA of the
-//       cluster (its own included) with st.async + a transaction-count mbarrier per (buffer, warp
-//       quadrant) — no fence, no cluster barrier.  w_(row,chunk) = 2^(z - Z_row) / L_row.
-//   pass C (one TMEM read):  acc_j += sum_i e_ij w_i   per-thread registers: with the 16x256b
+//       issued as two N <= 128 halves, each with its own full / empty barrier, so a half is
+//       refilled as soon as its column sums have been taken.
+//   The softmax is split over SPECIALISED warps (the v2 kernel ran both passes in the same warps
+//   and was bound by the latency of its own dependency chain, 2 warps per sub-partition):
+//   B warps (8: TMEM lane quadrant q x column half hf) — pass B, the only MUFU work.  One TMEM read,
+//       one write: a thread holds 2 rows x 16 columns of a 64-column chunk; it shifts by ITS OWN
+//       maximum of those 16 logits, rounded to an integer z (log2 domain): e = exp2(s c - z),
+//       written back in place; l += e.  No separate max pass, no shuffles inside the pass.  TMEM
+//       loads are double buffered.  Shifts per (thread, row, chunk) and (z, l) per (row, half) go
+//       to shared memory; B warps never wait for anything but the next S half.
+//   C warps (4: one per lane quadrant) — statistics and pass C.  (z, l) of a row are merged over
+//       the two halves and the CL CTAs with exact power-of-two rescaling built by integer
+//       arithmetic (no MUFU); across CTAs with st.async + a transaction-count mbarrier per
+//       (buffer, quadrant) — no fence, no cluster barrier.  w_(row,chunk) = 2^(z - Z_row) / L_row.
+//       pass C (one TMEM read):  acc_j += sum_i e_ij w_i  in per-thread registers: with the 16x256b
 //       TMEM load shape the column sum over ALL tiles of a segment is a plain packed FFMA2;
 //       lanes are combined once per segment.
 // TMEM holds two 128 x 256 fp32 S buffers (all 512 columns).  The K panel is double-buffered so a
 // segment change costs no bubble.
 //
-// Warp roles (640 threads): warps 0-15 softmax (WG g = warp/4 = 2 b + hf, 112 registers), 16 TMA
-// producer, 17 MMA issuer, 18-19 idle (32 registers; they complete the warpgroup whose registers
-// setmaxnreg hands to the softmax warps).
-// Output: partial[unit][2 p + b][j] (fp32), p = index of the range among those that touch the
-// unit; the select kernel sums the strips in fixed order, so scores are bit-reproducible run to
-// run (no atomics anywhere).
+// Warp roles (512 threads): warps 0-7 B (q = warp & 3, hf = warp >> 2), 8-11 C (q = warp & 3),
+// 12 TMA producer, 13 MMA issuer, 14-15 idle (they complete the warpgroup whose registers
+// setmaxnreg hands to the C warps).
+// Output: partial[unit][p][j] (fp32), p = index of the range among those that touch the unit;
+// the select kernel sums the strips in fixed order, so scores are bit-reproducible run to run
+// (no atomics anywhere).
 #include <cuda.h>
 
 #include <cstdio>
@@ -47,17 +49,16 @@ namespace kara {
 
 namespace {
 
-constexpr int kSoftmaxWarps = 16;
-constexpr int kProducerWarp = 16;
-constexpr int kMmaWarp = 17;
-constexpr int kThreads = 32 * 20;             // 5 warpgroups (setmaxnreg works per warpgroup); warps 18, 19 idle
-// setmaxnreg only moves registers inside the CTA's launch allocation (640 x 96; registers are
-// allocated per 4 warps, so 18 warps cost as much as 20): 512 x (112 - 96) <= 128 x (96 - 32)
-constexpr int kRegsSoftmax = 112, kRegsOther = 32;
+constexpr int kBWarps = 8;                    // pass B warps: 0..7
+constexpr int kCWarp0 = 8;                    // pass C warps: 8..11
+constexpr int kProducerWarp = 12;
+constexpr int kMmaWarp = 13;
+constexpr int kThreads = 32 * 16;             // 4 warpgroups (setmaxnreg works per warpgroup); warps 14, 15 idle
+// registers: 512 x 128 at launch; setmaxnreg moves them between warpgroups afterwards
+constexpr int kRegsC = 184, kRegsOther = 56;  // 128 x (184 - 128) <= 128 x (128 - 56)
 constexpr int kTileM = 128;
-constexpr int kKeysPerCta = 256;
-constexpr int kHalf = 128;                    // columns of one softmax warpgroup / of one MMA
-constexpr int kQStages = 2;
+constexpr int kKeysPerCta = 256;              // key rows (S columns) of one CTA = one TMEM buffer
+constexpr int kHalf = 128;                    // columns of one MMA half
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kMagic = 12582912.f;          // 1.5 * 2^23: x + kMagic rounds x to an integer in the low mantissa bits
@@ -114,6 +115,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       :: "r"(bar), "r"(parity) : "memory");
 }
 #endif
+// producer-side wait: polls with a pause, so the spinning warp does not take issue slots from the math warps
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  for (;;) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+    __nanosleep(64);
+  }
+}
 __device__ __forceinline__ uint32_t mapa(uint32_t local_addr, uint32_t cta) {
   uint32_t r;
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta));
@@ -127,6 +138,11 @@ __device__ __forceinline__ void st_async_b32x2(uint32_t cluster_addr, uint32_t a
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory");
 }
@@ -250,17 +266,19 @@ __device__ __forceinline__ float pow2i(int d) { return __int_as_float(max(d + 12
 template <int D, int CL>
 struct Smem {
   static constexpr int kPanels = D / 64;
-  static constexpr int kKStages = CL >= 4 ? 1 : 2;   // larger clusters need the room for the exchange slots
+  static constexpr int kKStages = CL >= 8 ? 1 : 2;   // 8-CTA clusters need the room for the exchange slots
+  static constexpr int kQStages = 2;
   static constexpr int kKBytes = kPanels * kKeysPerCta * 128;
   static constexpr int kQStageBytes = kPanels * kTileM * 128;
-  static constexpr int kParticipants = 2 * CL;       // (CTA, column half) pairs that own a piece of a row
   static constexpr int kOffK = 0;
   static constexpr int kOffQ = kOffK + kKStages * kKBytes;
-  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;            // float [16 warps][128]
-  static constexpr int kOffXch = kOffColsum + kSoftmaxWarps * kHalf * 4;        // uint2 [8 groups][2][2 CL][32]
-  static constexpr int kOffBars = kOffXch + 8 * 2 * kParticipants * 32 * 8;
-  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] xbar[8][2]  = 32 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 32 * 8;
+  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 C warps][256]
+  static constexpr int kOffZc = kOffColsum + 4 * kKeysPerCta * 4;        // int   [2 bufs][4 q][4 chunks][4 rows][32 lanes]
+  static constexpr int kOffRstat = kOffZc + 2 * 4 * 4 * 4 * 32 * 4;      // uint2 [2 bufs][2 halves][128 rows]
+  static constexpr int kOffXch = kOffRstat + 2 * 2 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
+  static constexpr int kOffBars = kOffXch + 2 * 4 * CL * 32 * 8;
+  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] = 26 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 26 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
@@ -300,71 +318,88 @@ __device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long 
   it.n_cols = max(16, (it.c_hi + 15) & ~15);
   return it;
 }
-// columns of half hf that the MMA produces (0 = the half is not computed at all)
-__device__ __forceinline__ int half_cols(const Seg& it, int hf) { return min(max(it.n_cols - hf * kHalf, 0), kHalf); }
+// columns the MMA of half hf produces (0 = half not issued)
+__device__ __forceinline__ int half_cols(int n_cols, int hf) { return min(max(n_cols - kHalf * hf, 0), kHalf); }
 
-// ---- pass B on one piece: 2 rows (K0, K0+1) x 16 columns of chunk C (of this half) held in r[32] ----
-// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column 64 C + 8 i + 2 qd + j (relative to the half).
-// Online softmax with exact power-of-two rescaling: the shift of this (row, chunk) is the running
-// maximum z = max(z_run, round(m c)) of the thread's integer shifts (log2 domain), so e <= 2^0.5;
-// l_run is rescaled by 2^(z_old - z) built from the exponent field (no MUFU).  Shifts are biased
-// ints (see kZFloor); a fully masked piece has m = -inf -> as_int(t) < 0 -> z = floor / z_run, e = 0.
-template <int C, int K0>
-__device__ __forceinline__ void pass_b_piece(uint32_t (&r)[32], int (&zc)[2][4], int (&zrun)[4], float (&lrun)[4],
-                                             float cs, int qd, int c_lo, int c_hi) {
-  constexpr int cb = C * 64;
-  if (!(cb >= c_lo && cb + 64 <= c_hi)) {   // warp-uniform: only the ragged first / last chunk
+// ---- pass B on one piece: 2 rows (K0, K0+1) x 16 columns of chunk CH (of this half) -----------------
+// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column col0 + 8 i + 2 qd + j of the CTA's 256; e gets the
+// exponentials in the same layout.  Online softmax with exact power-of-two rescaling: the shift of
+// this (row, chunk) is the running maximum z = max(z_run, round(m c)) of the thread's integer shifts
+// (log2 domain), so e <= 2^0.5; l_run is rescaled by 2^(z_old - z) built from the exponent field (no
+// MUFU).  Shifts are biased ints (see kZFloor); a fully masked piece has m = -inf -> as_int(t) < 0
+// -> z = floor / z_run, e = 0.
+template <int CH, int K0, bool RAGGED>
+__device__ __forceinline__ void pass_b_body(const uint32_t (&rin)[32], uint32_t (&e)[32], int (&zc)[2][4],
+                                            int (&zrun)[4], float (&lrun)[4], float cs, int qd, int col0,
+                                            int c_lo, int c_hi) {
+  float x[32];
+#pragma unroll
+  for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(rin[i]);
+  if (RAGGED) {
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const int col = cb + 8 * i + 2 * qd + j;
-        if (col < c_lo || col >= c_hi) { r[4 * i + j] = 0xff800000u; r[4 * i + 2 + j] = 0xff800000u; }
+        const int col = col0 + 8 * i + 2 * qd + j;
+        if (col < c_lo || col >= c_hi) { x[4 * i + j] = __int_as_float(0xff800000); x[4 * i + 2 + j] = __int_as_float(0xff800000); }
       }
     }
   }
-#define KARA_F(x) __uint_as_float(r[x])
-  float m0 = max3(KARA_F(0), KARA_F(1), KARA_F(4)), m1 = max3(KARA_F(2), KARA_F(3), KARA_F(6));
-  float m0b = max3(KARA_F(5), KARA_F(8), KARA_F(9)), m1b = max3(KARA_F(7), KARA_F(10), KARA_F(11));
-  m0 = max3(m0, KARA_F(12), KARA_F(13));   m1 = max3(m1, KARA_F(14), KARA_F(15));
-  m0b = max3(m0b, KARA_F(16), KARA_F(17)); m1b = max3(m1b, KARA_F(18), KARA_F(19));
-  m0 = max3(m0, KARA_F(20), KARA_F(21));   m1 = max3(m1, KARA_F(22), KARA_F(23));
-  m0b = max3(m0b, KARA_F(24), KARA_F(25)); m1b = max3(m1b, KARA_F(26), KARA_F(27));
-  m0 = max3(m0, KARA_F(28), KARA_F(29));   m1 = max3(m1, KARA_F(30), KARA_F(31));
-  m0 = fmaxf(m0, m0b);                     m1 = fmaxf(m1, m1b);
-#undef KARA_F
+  float m0 = max3(x[0], x[1], x[4]), m1 = max3(x[2], x[3], x[6]);
+  float m0b = max3(x[5], x[8], x[9]), m1b = max3(x[7], x[10], x[11]);
+  m0 = max3(m0, x[12], x[13]);   m1 = max3(m1, x[14], x[15]);
+  m0b = max3(m0b, x[16], x[17]); m1b = max3(m1b, x[18], x[19]);
+  m0 = max3(m0, x[20], x[21]);   m1 = max3(m1, x[22], x[23]);
+  m0b = max3(m0b, x[24], x[25]); m1b = max3(m1b, x[26], x[27]);
+  m0 = max3(m0, x[28], x[29]);   m1 = max3(m1, x[30], x[31]);
+  m0 = fmaxf(m0, m0b);           m1 = fmaxf(m1, m1b);
   // t = round(m c) + kMagic as a float; its bit pattern is the biased integer shift
   const float t0 = fminf(fmaf(m0, cs, kMagic), kMagic + kZLim);
   const float t1 = fminf(fmaf(m1, cs, kMagic), kMagic + kZLim);
-  const int z0 = max(zrun[K0], __float_as_int(t0)), z1 = max(zrun[K0 + 1], __float_as_int(t1));
+  int z0, z1;
   float l0s, l1s;
-  if (C == 0) { l0s = 0.f; l1s = 0.f; }     // first chunk of the tile: nothing accumulated yet
-  else { l0s = lrun[K0] * pow2i(zrun[K0] - z0); l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1); }
+  if (CH == 0) {                                 // first chunk of the tile: nothing accumulated yet
+    z0 = max(kZFloor, __float_as_int(t0)); z1 = max(kZFloor, __float_as_int(t1));
+    l0s = 0.f; l1s = 0.f;
+  } else {
+    z0 = max(zrun[K0], __float_as_int(t0)); z1 = max(zrun[K0 + 1], __float_as_int(t1));
+    l0s = lrun[K0] * pow2i(zrun[K0] - z0); l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
+  }
   zrun[K0] = z0; zrun[K0 + 1] = z1;
-  zc[C][K0] = z0; zc[C][K0 + 1] = z1;
+  zc[CH][K0] = z0; zc[CH][K0 + 1] = z1;
   const float nz0 = kMagic - __int_as_float(z0), nz1 = kMagic - __int_as_float(z1);   // = -z, exact
   const uint64_t cs2 = pk2(cs, cs), nz0_2 = pk2(nz0, nz0), nz1_2 = pk2(nz1, nz1);
   uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     float a, b;
-    upk2(fma2(pk2u(r[4 * i], r[4 * i + 1]), cs2, nz0_2), a, b);
+    upk2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
     a = ex2(a); b = ex2(b);
     l0 = add2(l0, pk2(a, b));
-    r[4 * i] = __float_as_uint(a); r[4 * i + 1] = __float_as_uint(b);
-    upk2(fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), cs2, nz1_2), a, b);
+    e[4 * i] = __float_as_uint(a); e[4 * i + 1] = __float_as_uint(b);
+    upk2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
     a = ex2(a); b = ex2(b);
     l1 = add2(l1, pk2(a, b));
-    r[4 * i + 2] = __float_as_uint(a); r[4 * i + 3] = __float_as_uint(b);
+    e[4 * i + 2] = __float_as_uint(a); e[4 * i + 3] = __float_as_uint(b);
   }
   float a, b;
   upk2(l0, a, b); lrun[K0] = a + b;
   upk2(l1, a, b); lrun[K0 + 1] = a + b;
 }
+// two copies of the body, so that the common (no ragged edge) path carries no select and no register copies
+template <int CH, int K0>
+__device__ __forceinline__ void pass_b_piece(const uint32_t (&rin)[32], uint32_t (&e)[32], int (&zc)[2][4],
+                                             int (&zrun)[4], float (&lrun)[4], float cs, int qd, int col0,
+                                             int c_lo, int c_hi) {
+  if (col0 >= c_lo && col0 + 64 <= c_hi)        // warp-uniform: false only on the ragged first / last chunk
+    pass_b_body<CH, K0, false>(rin, e, zc, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+  else
+    pass_b_body<CH, K0, true>(rin, e, zc, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+}
 
-// ---- pass C on one piece: acc[C*8 + i] (columns 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------------
+// ---- pass C on one piece: acc[C*8 + i] (columns 64 C + 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------
 template <int C, int K0>
-__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[16], const float (&w)[2][4]) {
+__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[32], const float (&w)[4][4]) {
   const uint64_t w0 = pk2(w[C][K0], w[C][K0]), w1 = pk2(w[C][K0 + 1], w[C][K0 + 1]);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
@@ -383,6 +418,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant__ CUtensorMap q_map,
                 const Call c, int T, int tpu, int tok_tiles) {
   using SM = Smem<D, CL>;
+  constexpr int QS = SM::kQStages;
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
@@ -390,10 +426,12 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t sK = base + SM::kOffK;
   const uint32_t sQ = base + SM::kOffQ;
   float* colsum = reinterpret_cast<float*>(gbase + SM::kOffColsum);
+  int* zcs = reinterpret_cast<int*>(gbase + SM::kOffZc);
+  uint2* rstat = reinterpret_cast<uint2*>(gbase + SM::kOffRstat);
   uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
   const uint32_t qfull = bars, qempty = bars + 16, kfull = bars + 32, kempty = bars + 48;
-  const uint32_t tfull = bars + 64, tempty = bars + 96, xbar = bars + 128;
+  const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -403,24 +441,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const long long g_end = (long long)(cluster_id + 1) * T / n_clusters;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < 2; ++i) {
-      mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1);
-      mbar_init(kfull + 8 * i, 1); mbar_init(kempty + 8 * i, 1);
-    }
+    for (int i = 0; i < 2; ++i) { mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(kfull + 8 * i, 1); mbar_init(kempty + 8 * i, 1); }
     for (int i = 0; i < 4; ++i) {
-      mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 4);   // one arrive per warp of the warpgroup
+      mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 4);   // one arrive per C warp
     }
-    for (int i = 0; i < 16; ++i) mbar_init(xbar + 8 * i, 2);       // per (buffer, warp quadrant) and parity: the two halves' warps arrive
+    for (int i = 0; i < 2; ++i) mbar_init(bdone + 8 * i, kBWarps);  // one arrive per B warp
+    for (int i = 0; i < 8; ++i) mbar_init(xbar + 8 * i, 1);        // per (buffer, quadrant)
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  cluster_sync_all();
+  if (CL > 1) cluster_sync_all();
   const uint32_t tmem_base = *tmem_ptr;
 
-  if (warp >= kSoftmaxWarps) {
+  if (warp >= kProducerWarp) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsOther));
   if (warp == kProducerWarp) {
     // ================================ TMA producer ==============================================
@@ -439,7 +476,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     auto load_k = [&](const Seg& it) {
       const int stage = k_iter % SM::kKStages, use = k_iter / SM::kKStages;
       ++k_iter;
-      mbar_wait(kempty + 8 * stage, (use & 1) ^ 1);
+      mbar_wait_backoff(kempty + 8 * stage, (use & 1) ^ 1);
       int my_bytes = 0, my_blk = -1, my_row = 0;
       if (lane < blocks_per_cta) {
         const int row0 = lane << c.g.bs_log2;                     // first panel row of this block in the CTA
@@ -474,8 +511,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       if (SM::kKStages == 2 && have_n) load_k(nxt);     // prefetch: its stage was released by the segment before `cur`
       if (lane == 0) {
         for (int tile = cur.t0; tile < cur.t1; ++tile, ++q_iter) {
-          const int stage = q_iter % kQStages, use = q_iter / kQStages;
-          mbar_wait(qempty + 8 * stage, (use & 1) ^ 1);
+          const int stage = q_iter % QS, use = q_iter / QS;
+          mbar_wait_backoff(qempty + 8 * stage, (use & 1) ^ 1);
           mbar_expect_tx(qfull + 8 * stage, SM::kQStageBytes);
           const int gq = tile / tok_tiles, tt = tile % tok_tiles;
           const int tok = (cur.li * c.n_seqs + cur.s) * c.W + c.q_row_begin + tt * kTileM;
@@ -492,111 +529,240 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     }
   } else if (warp == kMmaWarp) {
     // ================================ MMA issuer ================================================
-    if (lane == 0) {
-      int q_iter = 0, k_iter = 0, tile_iter = 0;
-      uint32_t t_par = 0;                      // bit (2 buf + hf): parity of the next use of that half buffer
-      for (long long g = g_begin; g < g_end;) {
+    // The whole warp walks the segments (warp-uniform values stay in uniform registers); one
+    // elected lane issues.  Descriptor low words are base + compile-time offsets: shared-memory
+    // addresses are < 2^18, so (addr >> 4) never carries out of the 14-bit address field.
+    constexpr uint32_t kDescHi = (uint32_t)(1024u >> 4) | (1u << 14) | (2u << 29);   // SBO | version | SWIZZLE_128B
+    constexpr uint32_t kDescLo = 1u << 16;                                           // LBO (unused)
+    int q_iter = 0, k_iter = 0, tile_iter = 0;
+    for (long long g = g_begin; g < g_end;) {
+      int n_tiles, n_cols;
+      {
         const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
-        g += it.t1 - it.t0;
-        if (!it.ok) continue;
-        const int nc0 = half_cols(it, 0), nc1 = half_cols(it, 1);
-        const int kstage = k_iter % SM::kKStages, kuse = k_iter / SM::kKStages;
-        ++k_iter;
-        mbar_wait(kfull + 8 * kstage, kuse & 1);
-        for (int tile = it.t0; tile < it.t1; ++tile, ++q_iter, ++tile_iter) {
-          const int stage = q_iter % kQStages, quse = q_iter / kQStages;
-          const int buf = tile_iter & 1;
-          mbar_wait(qfull + 8 * stage, quse & 1);
+        n_tiles = it.t1 - it.t0;
+        n_cols = it.ok ? it.n_cols : 0;
+      }
+      g += n_tiles;
+      if (n_cols == 0) continue;
+      const int kstage = k_iter % SM::kKStages, kuse = k_iter / SM::kKStages;
+      ++k_iter;
+      mbar_wait(kfull + 8 * kstage, kuse & 1);
+      const uint32_t b_lo = ((sK + kstage * SM::kKBytes) >> 4) | kDescLo;
+      for (int i = 0; i < n_tiles; ++i, ++q_iter, ++tile_iter) {
+        const int stage = q_iter % QS, quse = q_iter / QS;
+        const int buf = tile_iter & 1, tuse = tile_iter >> 1;
+        mbar_wait(qfull + 8 * stage, quse & 1);
+        const uint32_t a_lo = ((sQ + stage * SM::kQStageBytes) >> 4) | kDescLo;
 #pragma unroll
-          for (int hf = 0; hf < 2; ++hf) {
-            const int nc = hf ? nc1 : nc0;
-            if (nc == 0) continue;
-            const int slot = 2 * buf + hf;
-            mbar_wait(tempty + 8 * slot, ((t_par >> slot) & 1) ^ 1);
-            t_par ^= 1u << slot;
-            tc_fence_after();
-            const uint32_t d_tmem = tmem_base + buf * kKeysPerCta + hf * kHalf;
-            const uint32_t idesc = make_idesc_bf16(nc);
+        for (int hf = 0; hf < 2; ++hf) {
+          mbar_wait(tempty + 8 * (buf * 2 + hf), (tuse & 1) ^ 1);
+          tc_fence_after();
+          if (elect_one()) {
+            const int nc = half_cols(n_cols, hf);
+            if (nc > 0) {
+              const uint32_t idesc = make_idesc_bf16(nc);
+              const uint32_t d_tmem = tmem_base + buf * kKeysPerCta + hf * kHalf;
 #pragma unroll
-            for (int p = 0; p < SM::kPanels; ++p) {
+              for (int p = 0; p < SM::kPanels; ++p) {
 #pragma unroll
-              for (int ks = 0; ks < 4; ++ks) {
-                const uint64_t ad = make_sw128_desc(sQ + stage * SM::kQStageBytes + p * (kTileM * 128) + ks * 32);
-                const uint64_t bd = make_sw128_desc(sK + kstage * SM::kKBytes + p * (kKeysPerCta * 128) +
-                                                    hf * (kHalf * 128) + ks * 32);
-                umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
+                for (int ks = 0; ks < 4; ++ks) {
+                  const uint64_t ad = ((uint64_t)kDescHi << 32) | (a_lo + ((p * (kTileM * 128) + ks * 32) >> 4));
+                  const uint64_t bd = ((uint64_t)kDescHi << 32) |
+                                      (b_lo + ((p * (kKeysPerCta * 128) + hf * (kHalf * 128) + ks * 32) >> 4));
+                  umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
+                }
               }
             }
-            if (hf == 1 || nc1 == 0) umma_commit(qempty + 8 * stage);   // Q stage reusable once these MMAs have read it
-            umma_commit(tfull + 8 * slot);                               // this half of the S tile is complete
+            umma_commit(tfull + 8 * (buf * 2 + hf));   // S half complete (fires at once if nothing was issued)
+            if (hf == 1) {
+              umma_commit(qempty + 8 * stage);         // Q stage reusable once these MMAs have read it
+              if (i == n_tiles - 1) umma_commit(kempty + 8 * kstage);    // K stage reusable
+            }
           }
+          __syncwarp();
         }
-        umma_commit(kempty + 8 * kstage);    // K stage reusable
       }
     }
-    __syncwarp();
   }
-  } else {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsSoftmax));
-    // ================================ softmax warpgroups =========================================
-    constexpr int P = SM::kParticipants;
-    const int wg = warp >> 2, wq = warp & 3;
-    const int b = wg >> 1, hf = wg & 1;                 // TMEM buffer, column half
-    const int qd = lane & 3, lr = lane >> 2;            // column pair within a group of 8; row within 8
-    const int grp = b * 4 + wq;                         // exchange group: the warps that hold the same 32 rows
-    const float cs = kLog2e * rsqrtf((float)D);
-    const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + b * kKeysPerCta + hf * kHalf;
-    const uint32_t taddr_hi = taddr + (16u << 16);
-    const uint32_t tf = tfull + 8 * (2 * b + hf), te = tempty + 8 * (2 * b + hf);
-    uint64_t acc[16];
+  } else if (warp >= kCWarp0) {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsC));
+    // ================================ C warps: statistics + pass C ================================
+    const int q = warp & 3;                              // TMEM lane quadrant
+    const int qd = lane & 3, lr = lane >> 2;             // column pair within a group of 8; row within 8
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16);
+    uint64_t acc[32];
 #pragma unroll
-    for (int a = 0; a < 16; ++a) acc[a] = 0ull;
-    int tile_iter = 0, x_use = 0, t_use = 0;
+    for (int a = 0; a < 32; ++a) acc[a] = 0ull;
+    int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
-      float* out = c.partial + ((long long)it.unit * c.parts + 2 * it.part + b) * c.n_pad;
+      float* out = c.partial + ((long long)it.unit * c.parts + it.part) * c.n_pad;
       if (!it.ok) {
-        // skipped unit: its strips must still be defined (zeros); the status word says why
-        if (rank == 0 && hf == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
+        // skipped unit: its strip must still be defined (zeros); the status word says why
+        if (rank == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
         continue;
       }
-      const int n_chunks = (half_cols(it, hf) + 63) >> 6;                       // 0, 1 or 2
-      const int h_lo = min(max(it.c_lo - hf * kHalf, 0), kHalf), h_hi = min(max(it.c_hi - hf * kHalf, 0), kHalf);
+      const int n_chunks = (it.n_cols + 63) >> 6;                       // 1 .. 4
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        if ((tile_iter & 1) != b) continue;
-        const int use = x_use++;
+        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
+        mbar_wait(bdone + 8 * b, par);
+        // ---- row statistics (lane = row of this quadrant): two halves -> CTA -> cluster ----
+        int z_row;
+        float l_row;
+        {
+          const uint2 s0 = rstat[(b * 2 + 0) * 128 + q * 32 + lane], s1 = rstat[(b * 2 + 1) * 128 + q * 32 + lane];
+          z_row = max((int)s0.x, (int)s1.x);
+          l_row = __uint_as_float(s0.y) * pow2i((int)s0.x - z_row) + __uint_as_float(s1.y) * pow2i((int)s1.x - z_row);
+        }
+        if (CL > 1) {
+          // lane publishes its row to every peer CTA ...
+          const uint32_t bar = xbar + 8 * (b * 4 + q);
+          uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
+          if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
+          __syncwarp();
+          const uint32_t la = smem_u32(slot + rank * 32 + lane);
+#pragma unroll
+          for (int p = 0; p < CL; ++p)
+            if (p != rank) st_async_b32x2(mapa(la, p), (uint32_t)z_row, __float_as_uint(l_row), mapa(bar, p));
+          mbar_wait(bar, par);
+          // ... and merges that row over the CTAs in rank order (identical bits on every CTA)
+          int Z = z_row;
+#pragma unroll
+          for (int p = 0; p < CL; ++p) if (p != rank) Z = max(Z, (int)slot[p * 32 + lane].x);
+          float L = 0.f;
+#pragma unroll
+          for (int p = 0; p < CL; ++p) {
+            const uint2 v = slot[p * 32 + lane];
+            L += (p == rank) ? l_row * pow2i(z_row - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
+          }
+          z_row = Z; l_row = L;
+        }
+        const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + q * 32 + lane;
+        const float inv_row = (l_row > 0.f && tok < c.W) ? 1.f / l_row : 0.f;   // rows past the window contribute nothing
+        float w[4][4];
+        {
+          const int* zt = zcs + (size_t)((b * 4 + q) * 16) * 32 + lane;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const int zf = __shfl_sync(0xffffffffu, z_row, lr + 8 * k);
+            const float iv = __shfl_sync(0xffffffffu, inv_row, lr + 8 * k);
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch)
+              w[ch][k] = ch < n_chunks ? iv * pow2i(zt[(ch * 4 + k) * 32] - zf) : 0.f;
+          }
+        }
+        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
+        tc_fence_after();
+        const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
+        uint32_t ra[32], rb[32];
+        tmem_ld_16x256b_x8(ta, ra);
+        tmem_wait_ld();
+        tmem_ld_16x256b_x8(ta_hi, rb);
+        pass_c_piece<0, 0>(ra, acc, w);
+        tmem_wait_ld();
+        if (n_chunks > 1) tmem_ld_16x256b_x8(ta + 64, ra);
+        pass_c_piece<0, 2>(rb, acc, w);
+        if (n_chunks > 1) {
+          tmem_wait_ld();
+          tmem_ld_16x256b_x8(ta_hi + 64, rb);
+          pass_c_piece<1, 0>(ra, acc, w);
+          tmem_wait_ld();
+          if (n_chunks > 2) tmem_ld_16x256b_x8(ta + 128, ra);
+          pass_c_piece<1, 2>(rb, acc, w);
+        }
+        // half 0 has been read completely: the MMA may refill it
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 0));
+        if (n_chunks > 2) {
+          tmem_wait_ld();
+          tmem_ld_16x256b_x8(ta_hi + 128, rb);
+          pass_c_piece<2, 0>(ra, acc, w);
+          tmem_wait_ld();
+          if (n_chunks > 3) tmem_ld_16x256b_x8(ta + 192, ra);
+          pass_c_piece<2, 2>(rb, acc, w);
+          if (n_chunks > 3) {
+            tmem_wait_ld();
+            tmem_ld_16x256b_x8(ta_hi + 192, rb);
+            pass_c_piece<3, 0>(ra, acc, w);
+            tmem_wait_ld();
+            pass_c_piece<3, 2>(rb, acc, w);
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 1));
+      }
+
+      // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
+#pragma unroll
+      for (int a = 0; a < 32; ++a) {
+        float v0, v1;
+        upk2(acc[a], v0, v1);
+        v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
+        v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
+        v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
+        if (lr == 0)
+          *reinterpret_cast<float2*>(&colsum[q * kKeysPerCta + (a >> 3) * 64 + (a & 7) * 8 + 2 * qd]) = make_float2(v0, v1);
+        acc[a] = 0ull;
+      }
+      named_bar_sync(1, 128);
+#pragma unroll
+      for (int xx = 0; xx < 2; ++xx) {
+        const int x = (threadIdx.x & 127) + 128 * xx;
+        float v = 0.f;
+#pragma unroll
+        for (int wv = 0; wv < 4; ++wv) v += colsum[wv * kKeysPerCta + x];
+        if (x >= it.c_lo && x < it.c_hi) out[rank * kKeysPerCta + x - it.off] = v;
+      }
+      named_bar_sync(1, 128);
+    }
+  } else {
+    // ================================ B warps: pass B ================================================
+    const int q = warp & 3, hf = warp >> 2;              // TMEM lane quadrant; column half
+    const int qd = lane & 3, lr = lane >> 2;
+    const float cs = kLog2e * rsqrtf((float)D);
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + hf * kHalf;
+    int tile_iter = 0;
+    for (long long g = g_begin; g < g_end;) {
+      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+      g += it.t1 - it.t0;
+      if (!it.ok) continue;
+      const int n_ch = (half_cols(it.n_cols, hf) + 63) >> 6;            // chunks of this half: 0 .. 2
+      const int c_lo = it.c_lo, c_hi = it.c_hi;
+      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
+        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
         int zc[2][4], zq[4];
         float lq[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; }
-        uint32_t r[32];
-        if (n_chunks > 0) {
-          mbar_wait(tf, t_use & 1);
-          ++t_use;
-          tc_fence_after();
+        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; zc[0][k] = kZFloor; zc[1][k] = kZFloor; }
+        mbar_wait(tfull + 8 * (b * 2 + hf), par);
+        tc_fence_after();
+        if (n_ch > 0) {
           // ---- pass B: e = 2^(s c - z) in place; z per (row, chunk), running (z, l) per row ----
-          tmem_ld_16x256b_x8(taddr, r);
+          const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
+          uint32_t ra[32], rb[32], e[32];
+          tmem_ld_16x256b_x8(ta, ra);
           tmem_wait_ld();
-          pass_b_piece<0, 0>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
-          tmem_st_16x256b_x8(taddr, r);
-          tmem_ld_16x256b_x8(taddr_hi, r);
+          tmem_ld_16x256b_x8(ta_hi, rb);
+          pass_b_piece<0, 0>(ra, e, zc, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
+          tmem_st_16x256b_x8(ta, e);
           tmem_wait_ld();
-          pass_b_piece<0, 2>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
-          tmem_st_16x256b_x8(taddr_hi, r);
-          if (n_chunks > 1) {
-            tmem_ld_16x256b_x8(taddr + 64, r);
+          if (n_ch > 1) tmem_ld_16x256b_x8(ta + 64, ra);
+          pass_b_piece<0, 2>(rb, e, zc, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
+          tmem_st_16x256b_x8(ta_hi, e);
+          if (n_ch > 1) {
             tmem_wait_ld();
-            pass_b_piece<1, 0>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
-            tmem_st_16x256b_x8(taddr + 64, r);
-            tmem_ld_16x256b_x8(taddr_hi + 64, r);
+            tmem_ld_16x256b_x8(ta_hi + 64, rb);
+            pass_b_piece<1, 0>(ra, e, zc, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
+            tmem_st_16x256b_x8(ta + 64, e);
             tmem_wait_ld();
-            pass_b_piece<1, 2>(r, zc, zq, lq, cs, qd, h_lo, h_hi);
-            tmem_st_16x256b_x8(taddr_hi + 64, r);
+            pass_b_piece<1, 2>(rb, e, zc, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
+            tmem_st_16x256b_x8(ta_hi + 64, e);
           }
         }
-
-        // ---- row statistics: quad -> (CTA, half); then every (CTA, half) of the cluster -> row ----
+        // ---- row statistics of this half: quad -> row; shifts and (z, l) to shared memory ----
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const int zt = zq[k];
@@ -607,98 +773,20 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           lt += __shfl_xor_sync(0xffffffffu, lt, 2);
           zq[k] = zz; lq[k] = lt;
         }
-        float inv_row;
-        int z_row;
         {
-          // lane (lr, qd) publishes row lr + 8 qd of this warp to every CTA (its own included) ...
-          const int pb = use & 1;
-          const uint32_t bar = xbar + 8 * (grp * 2 + pb);
-          uint2* slot = xch + (size_t)(grp * 2 + pb) * P * 32;
-          const int zs = qd == 0 ? zq[0] : qd == 1 ? zq[1] : qd == 2 ? zq[2] : zq[3];
-          const float ls = qd == 0 ? lq[0] : qd == 1 ? lq[1] : qd == 2 ? lq[2] : lq[3];
-          const int row = lr + 8 * qd;
-          uint2* mine = slot + (rank * 2 + hf) * 32 + row;
-          *mine = make_uint2((uint32_t)zs, __float_as_uint(ls));              // own CTA: plain store + arrive
-          if (CL > 1) {
-            const uint32_t la = smem_u32(mine);
+          const int z_row = qd == 0 ? zq[0] : qd == 1 ? zq[1] : qd == 2 ? zq[2] : zq[3];
+          const float l_row = qd == 0 ? lq[0] : qd == 1 ? lq[1] : qd == 2 ? lq[2] : lq[3];
+          rstat[(b * 2 + hf) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
+          int* zt = zcs + (size_t)((b * 4 + q) * 16 + hf * 8) * 32 + lane;
 #pragma unroll
-            for (int p = 0; p < CL; ++p)
-              if (p != rank) st_async_b32x2(mapa(la, p), (uint32_t)zs, __float_as_uint(ls), mapa(bar, p));
-          }
-          __syncwarp();
-          if (lane == 0) {
-            if (CL > 1 && hf == 0) mbar_expect_tx(bar, (P - 2) * 32 * 8);    // the peers' bytes; counts as this warp's arrive
-            else mbar_arrive(bar);
-          }
-          mbar_wait(bar, (use >> 1) & 1);
-          // ... and merges that row over all participants (participant order: identical bits everywhere)
-          uint2 v[P];
+          for (int ch = 0; ch < 2; ++ch)
 #pragma unroll
-          for (int p = 0; p < P; ++p) v[p] = slot[p * 32 + row];
-          int Z = (int)v[0].x;
-#pragma unroll
-          for (int p = 1; p < P; ++p) Z = max(Z, (int)v[p].x);
-          float L = 0.f;
-#pragma unroll
-          for (int p = 0; p < P; ++p) L += __uint_as_float(v[p].y) * pow2i((int)v[p].x - Z);
-          const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + wq * 32 + row;
-          inv_row = (L > 0.f && tok < c.W) ? 1.f / L : 0.f;     // rows past the window contribute nothing
-          z_row = Z;
+            for (int k = 0; k < 4; ++k) zt[(ch * 4 + k) * 32] = zc[ch][k];
         }
-        if (n_chunks > 0) {
-          float w[2][4];
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const int zf = __shfl_sync(0xffffffffu, z_row, (lr << 2) | k);
-            const float iv = __shfl_sync(0xffffffffu, inv_row, (lr << 2) | k);
-            w[0][k] = iv * pow2i(zc[0][k] - zf);
-            w[1][k] = n_chunks > 1 ? iv * pow2i(zc[1][k] - zf) : 0.f;
-          }
-          // ---- pass C: acc_j += sum_i e_ij w_i ----
-          tmem_wait_st();
-          tmem_ld_16x256b_x8(taddr, r);
-          tmem_wait_ld();
-          pass_c_piece<0, 0>(r, acc, w);
-          tmem_ld_16x256b_x8(taddr_hi, r);
-          tmem_wait_ld();
-          pass_c_piece<0, 2>(r, acc, w);
-          if (n_chunks > 1) {
-            tmem_ld_16x256b_x8(taddr + 64, r);
-            tmem_wait_ld();
-            pass_c_piece<1, 0>(r, acc, w);
-            tmem_ld_16x256b_x8(taddr_hi + 64, r);
-            tmem_wait_ld();
-            pass_c_piece<1, 2>(r, acc, w);
-          }
-          // ---- release this half of the TMEM buffer to the MMA warp (all of this warp's reads have completed) ----
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(te);
-        }
-      }
-
-      // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
-      if (n_chunks > 0) {
-#pragma unroll
-        for (int a = 0; a < 16; ++a) {
-          float v0, v1;
-          upk2(acc[a], v0, v1);
-          v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
-          v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
-          v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
-          if (lr == 0)
-            *reinterpret_cast<float2*>(&colsum[warp * kHalf + (a >> 3) * 64 + (a & 7) * 8 + 2 * qd]) = make_float2(v0, v1);
-          acc[a] = 0ull;
-        }
-        named_bar_sync(1 + wg, 128);
-        {
-          const int x = threadIdx.x & 127;
-          float v = 0.f;
-#pragma unroll
-          for (int wv = 0; wv < 4; ++wv) v += colsum[(wg * 4 + wv) * kHalf + x];
-          if (x >= h_lo && x < h_hi) out[rank * kKeysPerCta + hf * kHalf + x - it.off] = v;
-        }
-        named_bar_sync(1 + wg, 128);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bdone + 8 * b);
       }
     }
   }
@@ -706,7 +794,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   // ---- teardown: nobody may exit while a peer can still write into this CTA ----
   tc_fence_before();
   __syncthreads();
-  cluster_sync_all();
+  if (CL > 1) cluster_sync_all();
   if (warp == kMmaWarp) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
 }
 
@@ -778,7 +866,7 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
   const long long per_range = T / n_clusters;
   long long ranges = (tpu - 1 + per_range - 1) / per_range + 1;
   if (ranges > tpu) ranges = tpu;
-  if (2 * ranges > c.parts) return tc_fail(KARA_ENOMEM, "workspace holds too few partial-score strips per unit");
+  if (kScoreStrips * ranges > c.parts) return tc_fail(KARA_ENOMEM, "workspace holds too few partial-score strips per unit");
 
   CUtensorMap kmap, qmap;
   memcpy(&kmap, s->k_map, sizeof kmap);
@@ -865,3 +953,4 @@ int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) 
 }
 
 }  // namespace kara
+
