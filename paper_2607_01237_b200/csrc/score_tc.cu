@@ -49,13 +49,14 @@ namespace kara {
 
 namespace {
 
-constexpr int kBWarps = 8;                    // pass B warps: 0..7
-constexpr int kCWarp0 = 8;                    // pass C warps: 8..11
-constexpr int kProducerWarp = 12;
-constexpr int kMmaWarp = 13;
-constexpr int kThreads = 32 * 16;             // 4 warpgroups (setmaxnreg works per warpgroup); warps 14, 15 idle
-// registers: 512 x 128 at launch; setmaxnreg moves them between warpgroups afterwards
-constexpr int kRegsC = 184, kRegsOther = 56;  // 128 x (184 - 128) <= 128 x (128 - 56)
+constexpr int kBWarps = 16;                   // pass B warps: 0..15
+constexpr int kCWarp0 = 16;                   // pass C warps: 16..19
+constexpr int kProducerWarp = 20;
+constexpr int kMmaWarp = 21;
+constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works per warpgroup); warps 22, 23 idle
+// registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
+// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, idle) = 6 x 80
+constexpr int kRegsB = 72, kRegsC = 152, kRegsOther = 40;
 constexpr int kTileM = 128;
 constexpr int kKeysPerCta = 256;              // key rows (S columns) of one CTA = one TMEM buffer
 constexpr int kHalf = 128;                    // columns of one MMA half
@@ -273,9 +274,9 @@ struct Smem {
   static constexpr int kOffK = 0;
   static constexpr int kOffQ = kOffK + kKStages * kKBytes;
   static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 C warps][256]
-  static constexpr int kOffZc = kOffColsum + 4 * kKeysPerCta * 4;        // int   [2 bufs][4 q][4 chunks][4 rows][32 lanes]
-  static constexpr int kOffRstat = kOffZc + 2 * 4 * 4 * 4 * 32 * 4;      // uint2 [2 bufs][2 halves][128 rows]
-  static constexpr int kOffXch = kOffRstat + 2 * 2 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
+  static constexpr int kOffZc = kOffColsum + 4 * kKeysPerCta * 4;        // short [2 bufs][4 q][4 chunks][4 rows][32 lanes] (unbiased shifts)
+  static constexpr int kOffRstat = kOffZc + 2 * 4 * 4 * 4 * 32 * 2;      // uint2 [2 bufs][4 chunks][128 rows]
+  static constexpr int kOffXch = kOffRstat + 2 * 4 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
   static constexpr int kOffBars = kOffXch + 2 * 4 * CL * 32 * 8;
   // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] = 26 x 8 B
   static constexpr int kOffTmemPtr = kOffBars + 26 * 8;
@@ -426,7 +427,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t sK = base + SM::kOffK;
   const uint32_t sQ = base + SM::kOffQ;
   float* colsum = reinterpret_cast<float*>(gbase + SM::kOffColsum);
-  int* zcs = reinterpret_cast<int*>(gbase + SM::kOffZc);
+  short* zcs = reinterpret_cast<short*>(gbase + SM::kOffZc);
   uint2* rstat = reinterpret_cast<uint2*>(gbase + SM::kOffRstat);
   uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
@@ -611,9 +612,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         int z_row;
         float l_row;
         {
-          const uint2 s0 = rstat[(b * 2 + 0) * 128 + q * 32 + lane], s1 = rstat[(b * 2 + 1) * 128 + q * 32 + lane];
-          z_row = max((int)s0.x, (int)s1.x);
-          l_row = __uint_as_float(s0.y) * pow2i((int)s0.x - z_row) + __uint_as_float(s1.y) * pow2i((int)s1.x - z_row);
+          uint2 sc[4];
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) sc[ch] = rstat[(b * 4 + ch) * 128 + q * 32 + lane];
+          z_row = max(max((int)sc[0].x, (int)sc[1].x), max((int)sc[2].x, (int)sc[3].x));
+          l_row = 0.f;
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) l_row += __uint_as_float(sc[ch].y) * pow2i((int)sc[ch].x - z_row);
         }
         if (CL > 1) {
           // lane publishes its row to every peer CTA ...
@@ -642,10 +647,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         const float inv_row = (l_row > 0.f && tok < c.W) ? 1.f / l_row : 0.f;   // rows past the window contribute nothing
         float w[4][4];
         {
-          const int* zt = zcs + (size_t)((b * 4 + q) * 16) * 32 + lane;
+          const short* zt = zcs + (size_t)((b * 4 + q) * 16) * 32 + lane;
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            const int zf = __shfl_sync(0xffffffffu, z_row, lr + 8 * k);
+            const int zf = __shfl_sync(0xffffffffu, z_row, lr + 8 * k) - kMagicBits;
             const float iv = __shfl_sync(0xffffffffu, inv_row, lr + 8 * k);
 #pragma unroll
             for (int ch = 0; ch < 4; ++ch)
@@ -720,49 +725,40 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     }
   } else {
     // ================================ B warps: pass B ================================================
-    const int q = warp & 3, hf = warp >> 2;              // TMEM lane quadrant; column half
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsB));
+    const int q = warp & 3, cq = warp >> 2, hf = cq >> 1;   // TMEM lane quadrant; 64-column chunk; MMA half of the chunk
     const int qd = lane & 3, lr = lane >> 2;
     const float cs = kLog2e * rsqrtf((float)D);
-    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + hf * kHalf;
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 64;
     int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
       if (!it.ok) continue;
-      const int n_ch = (half_cols(it.n_cols, hf) + 63) >> 6;            // chunks of this half: 0 .. 2
+      const bool active = cq * 64 < it.n_cols;              // the MMA writes this chunk
       const int c_lo = it.c_lo, c_hi = it.c_hi;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
         int zc[2][4], zq[4];
         float lq[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; zc[0][k] = kZFloor; zc[1][k] = kZFloor; }
+        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; zc[0][k] = kZFloor; }
         mbar_wait(tfull + 8 * (b * 2 + hf), par);
         tc_fence_after();
-        if (n_ch > 0) {
-          // ---- pass B: e = 2^(s c - z) in place; z per (row, chunk), running (z, l) per row ----
+        if (active) {
+          // ---- pass B: e = 2^(s c - z) in place; z per (thread, row), (z, l) per row ----
           const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
           uint32_t ra[32], rb[32], e[32];
           tmem_ld_16x256b_x8(ta, ra);
           tmem_wait_ld();
           tmem_ld_16x256b_x8(ta_hi, rb);
-          pass_b_piece<0, 0>(ra, e, zc, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
+          pass_b_piece<0, 0>(ra, e, zc, zq, lq, cs, qd, cq * 64, c_lo, c_hi);
           tmem_st_16x256b_x8(ta, e);
           tmem_wait_ld();
-          if (n_ch > 1) tmem_ld_16x256b_x8(ta + 64, ra);
-          pass_b_piece<0, 2>(rb, e, zc, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
+          pass_b_piece<0, 2>(rb, e, zc, zq, lq, cs, qd, cq * 64, c_lo, c_hi);
           tmem_st_16x256b_x8(ta_hi, e);
-          if (n_ch > 1) {
-            tmem_wait_ld();
-            tmem_ld_16x256b_x8(ta_hi + 64, rb);
-            pass_b_piece<1, 0>(ra, e, zc, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
-            tmem_st_16x256b_x8(ta + 64, e);
-            tmem_wait_ld();
-            pass_b_piece<1, 2>(rb, e, zc, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
-            tmem_st_16x256b_x8(ta_hi + 64, e);
-          }
         }
-        // ---- row statistics of this half: quad -> row; shifts and (z, l) to shared memory ----
+        // ---- row statistics of this chunk: quad -> row; shifts and (z, l) to shared memory ----
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const int zt = zq[k];
@@ -776,12 +772,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         {
           const int z_row = qd == 0 ? zq[0] : qd == 1 ? zq[1] : qd == 2 ? zq[2] : zq[3];
           const float l_row = qd == 0 ? lq[0] : qd == 1 ? lq[1] : qd == 2 ? lq[2] : lq[3];
-          rstat[(b * 2 + hf) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
-          int* zt = zcs + (size_t)((b * 4 + q) * 16 + hf * 8) * 32 + lane;
+          rstat[(b * 4 + cq) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
+          short* zt = zcs + (size_t)((b * 4 + q) * 16 + cq * 4) * 32 + lane;
 #pragma unroll
-          for (int ch = 0; ch < 2; ++ch)
-#pragma unroll
-            for (int k = 0; k < 4; ++k) zt[(ch * 4 + k) * 32] = zc[ch][k];
+          for (int k = 0; k < 4; ++k) zt[k * 32] = (short)(zc[0][k] - kMagicBits);
         }
         tmem_wait_st();
         tc_fence_before();
