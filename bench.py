@@ -73,6 +73,11 @@ def algorithmic(shape, L):
                 kv_in_bytes=shape.n_seqs * L * shape.W * shape.n_kv_heads * shape.head_dim * 2 * 2)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE score-kernel launch from the committed `ncu --set full`
+# capture (profiles/r1_v5b_ncu_cfg2.md), keyed by (workload, resident layers); None where no capture exists.
+NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40): 257.7e6 + 5.1e6}
+
+
 def _peaks():
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
@@ -107,7 +112,7 @@ class ClockSampler:
                 for bit, nm in self.REASONS.items():
                     if r & bit:
                         self.reasons.add(nm)
-                time.sleep(0.02)
+                time.sleep(0.005)
         except Exception as e:  # noqa: BLE001
             self.reasons.add(f"sampler_error:{type(e).__name__}")
 
@@ -305,7 +310,9 @@ def run_gpu(args):
         "gpu_launches": launches,
         "roofline": {"kernel": "score (a1)", "bound": "tensor", "achieved": achieved_tflops,
                      "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": achieved_tflops / peaks["bf16_tflops"],
-                     "traffic": None, "peak_source": peaks["source"] + ", burst bf16", "kernel_ms": sc_ms,
+                     "traffic": NCU_SCORE_TRAFFIC_BYTES.get((args.workload, L)),
+                     "traffic_source": "profiles/r1_v5b_ncu_cfg2.md (ncu --set full, dram rd+wr of one launch)",
+                     "peak_source": peaks["source"] + ", burst bf16", "kernel_ms": sc_ms,
                      "flops_per_launch": alg["flops"], "share_of_step": sc_ms / ms_per_step},
         "step_roofline": {"t_tensor_ms": t_tensor_ms, "t_hbm_ms": t_hbm_ms,
                           "frac": max(t_tensor_ms, t_hbm_ms) / ms_per_step,
