@@ -96,6 +96,7 @@ class ClockSampler:
     def __init__(self, index):
         self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
         self._stop = threading.Event()
+        self._ready = threading.Event()
         self._t = None
 
     def _loop(self):
@@ -112,13 +113,17 @@ class ClockSampler:
                 for bit, nm in self.REASONS.items():
                     if r & bit:
                         self.reasons.add(nm)
+                self._ready.set()
                 time.sleep(0.005)
         except Exception as e:  # noqa: BLE001
             self.reasons.add(f"sampler_error:{type(e).__name__}")
+            self._ready.set()
 
     def __enter__(self):
         self._t = threading.Thread(target=self._loop, daemon=True)
         self._t.start()
+        self._ready.wait(timeout=10)      # NVML is initialised and sampling before the timed region starts
+        self.samples.clear()
         return self
 
     def __exit__(self, *a):
@@ -180,10 +185,9 @@ def run_gpu(args):
     import torch
     from paper_2607_01237_b200 import inputs as kin
     from paper_2607_01237_b200 import kara
+    from paper_2607_01237_b200 import replicas
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local_rank, world = replicas.rank_env()
     dist = None
     if world > 1:
         import torch.distributed as dist_mod
@@ -195,7 +199,7 @@ def run_gpu(args):
 
     shape = _shape(args.workload)
     L = _resident_layers(args.workload, shape, args.layers)
-    seed = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}[args.workload] + 1000 * rank
+    seed = replicas.rank_seed({"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}[args.workload], rank)
     fill = "randn" if args.workload in ("cfg1", "cfg2") else "pattern"
     wl = kin.generate(shape, seed=seed, device=dev, n_layers_resident=L, history_fill=fill)
     alg = algorithmic(shape, L)
@@ -279,15 +283,10 @@ def run_gpu(args):
             e2e_s.append(dt)
     e2e_total = sum(e2e_s)
 
-    if dist:
-        t = torch.tensor([total_ms, e2e_total / len(e2e_s)], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_mean = float(t[0]), float(t[1])
-    else:
-        e2e_mean = e2e_total / len(e2e_s)
+    total_ms, e2e_mean = replicas.max_over_ranks([total_ms, e2e_total / len(e2e_s)], dist, dev)
 
     wc_step = shape.n_seqs * L                      # window-compressions per step per GPU
-    value = world * wc_step * args.steps / (total_ms * 1e-3)
+    value = replicas.job_throughput(world, wc_step, args.steps, total_ms)
     ms_per_step = total_ms / args.steps
     sc_ms = sum(score_ms) / len(score_ms)
     t_tensor_ms = alg["flops"] / (peaks["bf16_tflops"] * 1e12) * 1e3
@@ -320,7 +319,7 @@ def run_gpu(args):
     }
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
-            Ls = {"cfg1": 1, "cfg2": 10, "cfg3": 10, "cfg4": 3, "cfg5": 1}[args.workload]   # ~10-30 s of CPU work
+            Ls = {"cfg1": 1, "cfg2": 24, "cfg3": 24, "cfg4": 6, "cfg5": 2}[args.workload]   # ~10-30 s of CPU work
             small, H, desc = oracle_prepare(shape, Ls, seed=2)
             secs = oracle_leg(small, H, Ls)
             import multiprocessing

@@ -230,3 +230,65 @@ def test_gather_debug_logical_rows(gpu):
             np.testing.assert_array_equal(got, ref)
     fl = cache.gather_debug(kara.KARA_DBG_FREE_LIST, 0, 0, 0)
     np.testing.assert_array_equal(fl, wl.free_list[: int(wl.free_count)].numpy())
+
+
+def test_cfg2_full_size_sampled_units(gpu, oracle):
+    """BASELINE.json configs[1] at FULL size (40 layers x 8 KV heads = 320 units, 6,400 query tiles over
+    74 clusters: the launch configuration bench.py times).  The oracle is too slow for all of it, so:
+    properties on every unit (rows of a softmax sum to 1 => sum_j A_j = G W; F sorted, unique, in range;
+    closed-form lengths and freed-block count) and the full three-stage check on sampled units, each
+    computed one by one by the oracle from the logical rows."""
+    kara, gu = gpu
+    from oracle import kara_oracle as ko
+    from oracle import check
+    sh = kin.CFG2
+    wl = kin.generate(sh, seed=2)
+    D = gu.to_cuda(wl)
+    L, S, Hkv, G, n = sh.n_layers, sh.n_seqs, sh.n_kv_heads, sh.n_q_heads // sh.n_kv_heads, sh.W - sh.U
+    cache = kara.KaraCache(sh.block_size, L, Hkv, sh.head_dim)
+    cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+    cache.compress_window(0, L, D["bt"], D["sl"], D["ws"], D["q"], sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma,
+                          kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    assert cache.status() == 0 and cache.last_score_path() == 2
+    keep = ko.budget(n, sh.ratio)
+    assert keep == 96
+    h = int(wl.win_start[0]); old_len = int(wl.seq_lens[0]); t = old_len - h - sh.W
+    new_len = h + keep + sh.U + t
+    assert int(D["sl"][0]) == new_len
+    bs = sh.block_size
+    freed = -(-old_len // bs) - (-(-new_len // bs))
+    assert int(D["fc"][0]) - int(wl.free_count[0]) == freed
+    # ---- every unit: invariants ----
+    for l in range(L):
+        for hk in range(Hkv):
+            A = cache.gather_debug(kara.KARA_DBG_SCORES, l, 0, hk)
+            F = cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, 0, hk)
+            assert A.shape[0] == n and np.all(A > 0)
+            assert abs(float(A.astype(np.float64).sum()) - G * sh.W) <= 1e-4 * G * sh.W
+            assert F.shape[0] == keep and np.all(np.diff(F) > 0) and F[0] >= 0 and F[-1] < n
+    # ---- sampled units: S1 / S2 / S3 against the oracle, one unit at a time ----
+    rng = np.random.default_rng(7)
+    sample = {(0, 0), (L - 1, Hkv - 1)} | {(int(rng.integers(L)), int(rng.integers(Hkv))) for _ in range(6)}
+    n_amb = 0
+    for (l, hk) in sorted(sample):
+        q_bits = check.bits(wl.window_q[l, 0, :, hk * G:(hk + 1) * G, :])
+        k_old = check.bits(kin.logical_rows(wl.k_pool, l, wl.block_table[0], old_len, hk))
+        v_old = check.bits(kin.logical_rows(wl.v_pool, l, wl.block_table[0], old_len, hk))
+        A64, A32 = ko.scores(q_bits, k_old[h:h + n])
+        A = cache.gather_debug(kara.KARA_DBG_SCORES, l, 0, hk)
+        tol = check.score_tolerance(A64, G, sh.W, n)
+        assert np.all(np.abs(A.astype(np.float64) - A64) <= tol), f"S1 unit {(l, hk)}"
+        F = cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, 0, hk)
+        I = cache.gather_debug(kara.KARA_DBG_IDX_TOPK, l, 0, hk)
+        inj = ko.select(A, keep, sh.alpha, sh.gamma)                 # S2: oracle on the GPU's own scores
+        np.testing.assert_array_equal(I, inj["I"])
+        np.testing.assert_array_equal(F, inj["F"])
+        for what, old in ((kara.KARA_DBG_K_LOGICAL, k_old), (kara.KARA_DBG_V_LOGICAL, v_old)):
+            got = cache.gather_debug(what, l, 0, hk, D["bt"], D["sl"])
+            np.testing.assert_array_equal(got, ko.compact_rows(old, h, sh.W, sh.U, t, F))
+        own = ko.select(A32, keep, sh.alpha, sh.gamma)               # S3
+        if not np.array_equal(F, own["F"]):
+            assert check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 hard mismatch at unit {(l, hk)}"
+            n_amb += 1
+    assert n_amb <= len(sample)
