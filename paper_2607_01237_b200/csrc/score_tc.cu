@@ -644,7 +644,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           z_row = Z; l_row = L;
         }
         const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + q * 32 + lane;
-        const float inv_row = (l_row > 0.f && tok < c.W) ? 1.f / l_row : 0.f;   // rows past the window contribute nothing
+        const float inv_row = (l_row > 0.f && tok < c.W) ? __fdividef(1.f, l_row) : 0.f;   // rows past the window contribute nothing
         float w[4][4];
         {
           const short* zt = zcs + (size_t)((b * 4 + q) * 16) * 32 + lane;
@@ -759,24 +759,35 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           tmem_st_16x256b_x8(ta_hi, e);
         }
         // ---- row statistics of this chunk: quad -> row; shifts and (z, l) to shared memory ----
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const int zt = zq[k];
-          int zz = max(zt, __shfl_xor_sync(0xffffffffu, zt, 1));
-          zz = max(zz, __shfl_xor_sync(0xffffffffu, zz, 2));
-          float lt = lq[k] * pow2i(zt - zz);
-          lt += __shfl_xor_sync(0xffffffffu, lt, 1);
-          lt += __shfl_xor_sync(0xffffffffu, lt, 2);
-          zq[k] = zz; lq[k] = lt;
-        }
         {
-          const int z_row = qd == 0 ? zq[0] : qd == 1 ? zq[1] : qd == 2 ? zq[2] : zq[3];
-          const float l_row = qd == 0 ? lq[0] : qd == 1 ? lq[1] : qd == 2 ? lq[2] : lq[3];
-          rstat[(b * 4 + cq) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
           short* zt = zcs + (size_t)((b * 4 + q) * 16 + cq * 4) * 32 + lane;
 #pragma unroll
           for (int k = 0; k < 4; ++k) zt[k * 32] = (short)(zc[0][k] - kMagicBits);
         }
+        // reduce-scatter over the 4 lanes of a quad: lane qd ends up with row k = qd (6 shuffles)
+        int z_row;
+        float l_row;
+        {
+          const bool p1 = qd & 1, p2 = qd & 2;
+          // step 1 (lane ^ 1): keep rows {p1, p1 + 2}, hand the other two over
+          const int ks0 = p1 ? zq[1] : zq[0], ks1 = p1 ? zq[3] : zq[2];
+          const float kl0 = p1 ? lq[1] : lq[0], kl1 = p1 ? lq[3] : lq[2];
+          const int rz0 = __shfl_xor_sync(0xffffffffu, p1 ? zq[0] : zq[1], 1);
+          const int rz1 = __shfl_xor_sync(0xffffffffu, p1 ? zq[2] : zq[3], 1);
+          const float rl0 = __shfl_xor_sync(0xffffffffu, p1 ? lq[0] : lq[1], 1);
+          const float rl1 = __shfl_xor_sync(0xffffffffu, p1 ? lq[2] : lq[3], 1);
+          const int za = max(ks0, rz0), zb = max(ks1, rz1);
+          const float la = kl0 * pow2i(ks0 - za) + rl0 * pow2i(rz0 - za);
+          const float lb = kl1 * pow2i(ks1 - zb) + rl1 * pow2i(rz1 - zb);
+          // step 2 (lane ^ 2): keep row p1 + 2 p2 = qd
+          const int kz = p2 ? zb : za;
+          const float kl = p2 ? lb : la;
+          const int rz = __shfl_xor_sync(0xffffffffu, p2 ? za : zb, 2);
+          const float rl = __shfl_xor_sync(0xffffffffu, p2 ? la : lb, 2);
+          z_row = max(kz, rz);
+          l_row = kl * pow2i(kz - z_row) + rl * pow2i(rz - z_row);
+        }
+        rstat[(b * 4 + cq) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
