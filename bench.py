@@ -207,7 +207,7 @@ def run_gpu(args):
 
     cache = kara.KaraCache(shape.block_size, L, shape.n_kv_heads, shape.head_dim)
     cache.attach_pool(wl.k_pool, wl.v_pool, wl.free_list, wl.free_count)
-    cache.enable_score_timing(True)
+    cache.enable_score_timing(not args.no_score_timing)
     flags = kara.KARA_COMMIT | (kara.KARA_SCORE_SIMT if args.simt else 0)
     ws = torch.empty(cache.workspace_bytes(L, shape.n_seqs, shape.n_q_heads, shape.W, shape.U, shape.ratio,
                                            shape.alpha), dtype=torch.uint8, device=dev)
@@ -340,6 +340,8 @@ def main():
     ap.add_argument("--layers", type=int, default=0, help="resident layers (default: all that fit)")
     ap.add_argument("--simt", action="store_true", help="force the CUDA-core score kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-score-timing", action="store_true",
+                    help="no CUDA events inside the library around the score launch (roofline.kernel_ms = 0)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -18,6 +18,7 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
   __shared__ int warp_tot[kThreads / 32];
   __shared__ int s_running;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // launched programmatically behind select_compact
   if (tid == 0) s_running = *c.free_count;
   __syncthreads();
   for (int s0 = 0; s0 < c.n_seqs; s0 += kThreads) {
@@ -89,8 +90,14 @@ __global__ void gather_rows_kernel(Geom g, const __nv_bfloat16* pool, int layer,
 }  // namespace
 
 cudaError_t launch_metadata(const Call& c, cudaStream_t st) {
-  metadata_kernel<<<1, kThreads, 0, st>>>(c);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg{};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cfg.gridDim = dim3(1); cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  return cudaLaunchKernelEx(&cfg, metadata_kernel, c);
 }
 
 cudaError_t launch_gather_rows(const Geom& g, const __nv_bfloat16* pool, int layer, int kv_head,

@@ -457,6 +457,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   tc_fence_after();
   if (CL > 1) cluster_sync_all();
   const uint32_t tmem_base = *tmem_ptr;
+  // programmatic dependent launch: the select/compaction grid may be scheduled as SMs drain (it waits for
+  // this whole grid with griddepcontrol.wait before it reads anything)
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   if (warp >= kProducerWarp) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsOther));

@@ -149,7 +149,11 @@ __device__ __forceinline__ void st_na16(void* p, const uint4& v) {
                :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-__global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, int stage_rows) {
+__global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, int stage_rows, int off_bytes) {
+  // programmatic dependent launch: this grid may be scheduled while the score kernel drains; nothing the
+  // score kernel writes is read before the wait, and the metadata kernel behind may be scheduled early too
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = c.n, n_pad = c.n_pad, k = c.k, keep = c.keep, d = c.g.d;
   // carve
@@ -164,6 +168,7 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
   unsigned char* s_sel = reinterpret_cast<unsigned char*>(sc + 1);             // [n_pad] retained flag
   unsigned char* s_csel = s_sel + n_pad;                                       // [k_pad] chunk flags
   unsigned char* s_celig = s_csel + c.k_pad;                                   // [k_pad]
+  long long* s_off = reinterpret_cast<long long*>(smem_raw + off_bytes);       // [2][stage_rows] src / dst offsets
 
   const int unit = blockIdx.x, tid = threadIdx.x;
   int li, s, hk;
@@ -243,16 +248,25 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
     __nv_bfloat16* pool = const_cast<__nv_bfloat16*>(which == 0 ? c.k_pool : c.v_pool);
     for (int c0 = 0; c0 < moved; c0 += stage_rows) {
       const int rows = min(stage_rows, moved - c0);
+      // the block-table walk once per row (the same for K and V), not once per 16-byte vector
+      if (which == 0 || moved > stage_rows) {
+        for (int r = tid; r < rows; r += kThreads) {
+          const int row = c0 + r;
+          const int src = row < keep ? h + s_F[row] : h + n + (row - keep);
+          s_off[r] = row_offset(c, layer, s, hk, src);
+          s_off[stage_rows + r] = row_offset(c, layer, s, hk, h + row);
+        }
+        __syncthreads();
+      }
       for (int x = tid; x < rows * vpr; x += kThreads) {
-        const int row = c0 + x / vpr, v = x % vpr;
-        const int src = row < keep ? h + s_F[row] : h + n + (row - keep);
-        const long long off = row_offset(c, layer, s, hk, src);
+        const int r = x / vpr, v = x % vpr;
+        const long long off = s_off[r];
         s_stage[x] = off >= 0 ? ld_stream16(pool + off + v * 8) : make_uint4(0, 0, 0, 0);
       }
       __syncthreads();
       for (int x = tid; x < rows * vpr; x += kThreads) {
-        const int row = c0 + x / vpr, v = x % vpr;
-        const long long off = row_offset(c, layer, s, hk, h + row);
+        const int r = x / vpr, v = x % vpr;
+        const long long off = s_off[stage_rows + r];
         if (off >= 0) st_na16(pool + off + v * 8, s_stage[x]);
       }
       __syncthreads();
@@ -266,7 +280,7 @@ size_t smem_bytes(const Call& c, int stage_rows) {
   b += sizeof(int) * (c.k_pad + c.keep_pad) + sizeof(unsigned) * c.k_pad;
   b += sizeof(Scratch);
   b += (size_t)c.n_pad + 2 * (size_t)c.k_pad;
-  return (b + 15) / 16 * 16;
+  return (b + 15) / 16 * 16;   // the row-offset table [2][stage_rows] of int64 follows at this offset
 }
 
 }  // namespace
@@ -280,11 +294,19 @@ cudaError_t launch_select_compact(const Call& c, cudaStream_t st) {
   if (stage_rows > cap_rows) stage_rows = cap_rows;
   // the staging area doubles as the fill-flag array (n bytes)
   if (stage_rows * rowB < c.n_pad) stage_rows = (c.n_pad + rowB - 1) / rowB;
-  const size_t smem = smem_bytes(c, stage_rows);
+  const size_t off_bytes = smem_bytes(c, stage_rows);
+  const size_t smem = off_bytes + 2 * sizeof(long long) * (size_t)stage_rows;
   cudaError_t e = cudaFuncSetAttribute(select_compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  select_compact_kernel<<<units, kThreads, smem, st>>>(c, stage_rows);
-  return cudaGetLastError();
+  // programmatic dependent launch behind the score kernel (see the kernel's first lines)
+  cudaLaunchConfig_t cfg{};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cfg.gridDim = dim3(units); cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  return cudaLaunchKernelEx(&cfg, select_compact_kernel, c, stage_rows, (int)off_bytes);
 }
 
 }  // namespace kara
