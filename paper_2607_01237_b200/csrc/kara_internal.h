@@ -115,6 +115,5 @@ cudaError_t launch_metadata(const Call& c, cudaStream_t st);
 cudaError_t launch_gather_rows(const Geom& g, const __nv_bfloat16* pool, int layer, int kv_head,
                                const int32_t* bt_row, int length, __nv_bfloat16* out, int32_t* status,
                                cudaStream_t st);
-size_t select_compact_smem_bytes(const Call& c, int moved_rows_hint);
 
 }  // namespace kara

@@ -12,9 +12,9 @@
 // index order with a ballot-free segmented count + block scan.  All decisions are integer
 // compares on fp32 bit patterns, so the result is a pure function of the scores.
 //
-// In-place compaction is hazard-free with one CTA per (unit, tensor): destination c <= source
-// F[c] and both are increasing, so staging rows [c0,c1) in shared memory, barrier, then writing
-// them never overwrites a row a later chunk still has to read.
+// In-place compaction is hazard-free with one CTA per unit: destination c <= source F[c] and both
+// are increasing, so loading rows [c0,c1) into registers, barrier, then writing them never
+// overwrites a row a later chunk still has to read.
 #include "kara_internal.h"
 
 namespace kara {
@@ -149,7 +149,7 @@ __device__ __forceinline__ void st_na16(void* p, const uint4& v) {
                :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-__global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, int stage_rows, int off_bytes) {
+__global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call c, int stage_rows, int off_bytes) {
   // programmatic dependent launch: this grid may be scheduled while the score kernel drains; nothing the
   // score kernel writes is read before the wait, and the metadata kernel behind may be scheduled early too
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -157,9 +157,9 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = c.n, n_pad = c.n_pad, k = c.k, keep = c.keep, d = c.g.d;
   // carve
-  uint4* s_stage = reinterpret_cast<uint4*>(smem_raw);                         // [stage_rows][d*2/16]
+  unsigned char* s_fill = smem_raw;                                            // [n_pad] fill flags
   const int vpr = d / 8;                                                       // 16-byte vectors per row
-  float* s_A = reinterpret_cast<float*>(s_stage + (size_t)stage_rows * vpr);   // [n_pad]
+  float* s_A = reinterpret_cast<float*>(smem_raw + ((n_pad + 15) / 16) * 16);  // [n_pad]
   unsigned* s_key = reinterpret_cast<unsigned*>(s_A + n_pad);                  // [n_pad]
   int* s_I = reinterpret_cast<int*>(s_key + n_pad);                            // [k_pad]
   int* s_F = s_I + c.k_pad;                                                    // [keep_pad]
@@ -213,10 +213,19 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
   block_excl_scan(n_elig_local, sc, &n_elig);
   __syncthreads();
   const int n_pick = min(c.P, n_elig);
-  {
-    const unsigned char* elig = s_celig;
-    block_top_m(s_rkey, k - 1, n_pick, [elig](int x) { return elig[x] != 0; }, s_csel, sc);
+  // top-P of the (few) eligible chunks under (R desc, ordinal asc) by direct ranking: a chunk is picked
+  // iff fewer than n_pick eligible chunks precede it in that order
+  for (int x = tid; x < k - 1; x += kThreads) {
+    if (!s_celig[x]) continue;
+    const unsigned rx = s_rkey[x];
+    int before = 0;
+    for (int y = 0; y < k - 1; ++y) {
+      const unsigned ry = s_rkey[y];
+      before += (s_celig[y] && (ry > rx || (ry == rx && y < x))) ? 1 : 0;
+    }
+    if (before < n_pick) s_csel[x] = 1;
   }
+  __syncthreads();
   int added_local = 0;
   for (int x = tid; x < k - 1; x += kThreads)
     if (s_csel[x]) {
@@ -229,10 +238,10 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
   // ---- App. C.3 fill --------------------------------------------------------------------------
   {
     // Candidates are the positions unselected before the fill.  The histogram passes need a
-    // stable candidate set, so the fill selects into its own flag array (the staging area is
-    // free until a4) and the flags are merged afterwards.
+    // stable candidate set, so the fill selects into its own flag array and the flags are merged
+    // afterwards.
     const unsigned char* selc = s_sel;
-    unsigned char* fillflag = reinterpret_cast<unsigned char*>(s_stage);
+    unsigned char* fillflag = s_fill;
     for (int j = tid; j < n; j += kThreads) fillflag[j] = 0;
     __syncthreads();
     block_top_m(s_key, n, keep - k - added, [selc](int j) { return selc[j] == 0; }, fillflag, sc);
@@ -242,40 +251,49 @@ __global__ void __launch_bounds__(kThreads) select_compact_kernel(const Call c, 
   block_compact(s_sel, n, s_F, sc);   // F: ascending (reading G10), |F| = keep
   if (c.keep_debug) for (int x = tid; x < keep; x += kThreads) c.idx_final[(long long)unit * c.keep_pad + x] = s_F[x];
 
-  // ---- a4: compaction of K then V (Eq. 9), staged through shared memory ------------------------
+  // ---- a4: compaction of K and V (Eq. 9), staged through REGISTERS -----------------------------
+  // A chunk of kRowsPerPass rows of K and of V is loaded completely (every thread holds its 16-byte
+  // vectors in registers: all loads of the chunk are in flight together), the block synchronises, then
+  // the chunk is written.  Destination row c <= source row F[c], both increasing, so a chunk's writes
+  // never touch a row a later chunk still has to read.
   const int moved = keep + c.U + t;
-  for (int which = 0; which < 2; ++which) {
-    __nv_bfloat16* pool = const_cast<__nv_bfloat16*>(which == 0 ? c.k_pool : c.v_pool);
-    for (int c0 = 0; c0 < moved; c0 += stage_rows) {
-      const int rows = min(stage_rows, moved - c0);
-      // the block-table walk once per row (the same for K and V), not once per 16-byte vector
-      if (which == 0 || moved > stage_rows) {
-        for (int r = tid; r < rows; r += kThreads) {
-          const int row = c0 + r;
-          const int src = row < keep ? h + s_F[row] : h + n + (row - keep);
-          s_off[r] = row_offset(c, layer, s, hk, src);
-          s_off[stage_rows + r] = row_offset(c, layer, s, hk, h + row);
-        }
-        __syncthreads();
-      }
-      for (int x = tid; x < rows * vpr; x += kThreads) {
-        const int r = x / vpr, v = x % vpr;
-        const long long off = s_off[r];
-        s_stage[x] = off >= 0 ? ld_stream16(pool + off + v * 8) : make_uint4(0, 0, 0, 0);
-      }
-      __syncthreads();
-      for (int x = tid; x < rows * vpr; x += kThreads) {
-        const int r = x / vpr, v = x % vpr;
-        const long long off = s_off[stage_rows + r];
-        if (off >= 0) st_na16(pool + off + v * 8, s_stage[x]);
-      }
-      __syncthreads();
+  constexpr int kVecPerThread = 8;                             // per tensor
+  const int rows_per_pass = kThreads * kVecPerThread / vpr;    // 128 rows at d = 128, 256 at d = 64
+  __nv_bfloat16* kp = const_cast<__nv_bfloat16*>(c.k_pool);
+  __nv_bfloat16* vp = const_cast<__nv_bfloat16*>(c.v_pool);
+  for (int c0 = 0; c0 < moved; c0 += rows_per_pass) {
+    const int rows = min(rows_per_pass, moved - c0);
+    // the block-table walk once per row (the same for K and V), not once per 16-byte vector
+    for (int r = tid; r < rows; r += kThreads) {
+      const int row = c0 + r;
+      const int src = row < keep ? h + s_F[row] : h + n + (row - keep);
+      s_off[r] = row_offset(c, layer, s, hk, src);
+      s_off[stage_rows + r] = row_offset(c, layer, s, hk, h + row);
     }
+    __syncthreads();
+    uint4 kv[kVecPerThread], vv[kVecPerThread];
+#pragma unroll
+    for (int u = 0; u < kVecPerThread; ++u) {
+      const int x = tid + u * kThreads;
+      const int r = x / vpr, v = x % vpr;
+      const long long off = r < rows ? s_off[r] : -1;
+      kv[u] = off >= 0 ? __ldcg(reinterpret_cast<const uint4*>(kp + off + v * 8)) : make_uint4(0, 0, 0, 0);
+      vv[u] = off >= 0 ? __ldcg(reinterpret_cast<const uint4*>(vp + off + v * 8)) : make_uint4(0, 0, 0, 0);
+    }
+    __syncthreads();                                           // every read of the chunk has completed
+#pragma unroll
+    for (int u = 0; u < kVecPerThread; ++u) {
+      const int x = tid + u * kThreads;
+      const int r = x / vpr, v = x % vpr;
+      const long long off = r < rows ? s_off[stage_rows + r] : -1;
+      if (off >= 0) { st_na16(kp + off + v * 8, kv[u]); st_na16(vp + off + v * 8, vv[u]); }
+    }
+    __syncthreads();
   }
 }
 
-size_t smem_bytes(const Call& c, int stage_rows) {
-  size_t b = (size_t)stage_rows * c.g.d * 2;
+size_t smem_bytes(const Call& c) {
+  size_t b = (size_t)((c.n_pad + 15) / 16) * 16;
   b += sizeof(float) * c.n_pad + sizeof(unsigned) * c.n_pad;
   b += sizeof(int) * (c.k_pad + c.keep_pad) + sizeof(unsigned) * c.k_pad;
   b += sizeof(Scratch);
@@ -287,14 +305,9 @@ size_t smem_bytes(const Call& c, int stage_rows) {
 
 cudaError_t launch_select_compact(const Call& c, cudaStream_t st) {
   const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;
-  // stage the whole moved range when it fits (keep + U + a little tail), else chunk
-  const int rowB = c.g.d * 2;
-  int stage_rows = c.keep + c.U + 2 * c.g.bs;
-  const int cap_rows = (160 * 1024) / rowB;
-  if (stage_rows > cap_rows) stage_rows = cap_rows;
-  // the staging area doubles as the fill-flag array (n bytes)
-  if (stage_rows * rowB < c.n_pad) stage_rows = (c.n_pad + rowB - 1) / rowB;
-  const size_t off_bytes = smem_bytes(c, stage_rows);
+  // offset table: one pass of the compaction moves 256 x 8 vectors per tensor = at most 256 rows (d = 64)
+  const int stage_rows = 256;
+  const size_t off_bytes = smem_bytes(c);
   const size_t smem = off_bytes + 2 * sizeof(long long) * (size_t)stage_rows;
   cudaError_t e = cudaFuncSetAttribute(select_compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
