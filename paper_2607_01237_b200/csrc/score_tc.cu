@@ -68,6 +68,10 @@ constexpr int kMagicBits = 0x4B400000;
 // are clamped to z <= kZLim (|logit| log2e / sqrt(d) beyond that is not served) and floored at
 // -kZLim, which is also the shift of a piece with no valid key (its l is 0)
 constexpr float kZLim = 32000.f;
+#ifndef KARA_POLY_MASK
+#define KARA_POLY_MASK 0x00                   // bit i: column group i of 8 uses the FMA-pipe polynomial (measured: 0x52 is 7 % slower)
+#endif
+constexpr unsigned kPolyMask = KARA_POLY_MASK;
 constexpr int kZFloor = kMagicBits - 32000;
 
 char g_tc_err[256] = "";
@@ -258,6 +262,28 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
   return r;
 }
+// 2^x for a pair of x <= 0.5 on the FMA pipe (the MUFU pipe, 16 ex2/clk/SM, is the scarcer resource
+// of pass B: one ex2 per 2 d tensor FLOPs): x = n + f, n = round(x) by the magic-number add, f in
+// [-0.5, 0.5]; 2^f by a degree-3 polynomial (relative minimax fit, max error 7.5e-5 in fp32 Horner,
+// far inside the 1e-3 score tolerance); 2^n by adding n to the exponent field.
+constexpr float kP0 = 0.9999281168f, kP1 = 0.6932609677f, kP2 = 0.2426105440f, kP3 = 0.0551713221f;
+__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& a, float& b) {
+  float xa, xb;
+  upk2(x2, xa, xb);
+  xa = fmaxf(xa, -125.f); xb = fmaxf(xb, -125.f);          // below fp32's normal range: 2^-125 stands in for 0
+  const uint64_t xc = pk2(xa, xb);
+  const uint64_t t2 = add2(xc, pk2(kMagic, kMagic));         // low mantissa bits = round(x)
+  const uint64_t n2 = add2(t2, pk2(-kMagic, -kMagic));       // round(x) as a float, exact
+  const uint64_t f2 = fma2(n2, pk2(-1.f, -1.f), xc);         // x - round(x), exact
+  uint64_t p2 = fma2(pk2(kP3, kP3), f2, pk2(kP2, kP2));
+  p2 = fma2(p2, f2, pk2(kP1, kP1));
+  p2 = fma2(p2, f2, pk2(kP0, kP0));
+  float pa, pb, ta, tb;
+  upk2(p2, pa, pb);
+  upk2(t2, ta, tb);
+  a = __int_as_float(__float_as_int(pa) + (__float_as_int(ta) << 23));
+  b = __int_as_float(__float_as_int(pb) + (__float_as_int(tb) << 23));
+}
 // 2^d for d <= 0 built from the exponent field; 0 for d <= -127 (such weights are below fp32's range)
 __device__ __forceinline__ float pow2i(int d) { return __int_as_float(max(d + 127, 0) << 23); }
 
@@ -373,13 +399,16 @@ __device__ __forceinline__ void pass_b_body(const uint32_t (&rin)[32], uint32_t 
   uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
+    // kPolyMask: column groups whose exponentials run on the FMA pipe (never on a ragged chunk,
+    // where masked columns must come out as exact zeros)
+    const bool poly = !RAGGED && ((kPolyMask >> i) & 1);
     float a, b;
-    upk2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
-    a = ex2(a); b = ex2(b);
+    if (poly) exp2_poly2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
+    else { upk2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b); a = ex2(a); b = ex2(b); }
     l0 = add2(l0, pk2(a, b));
     e[4 * i] = __float_as_uint(a); e[4 * i + 1] = __float_as_uint(b);
-    upk2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
-    a = ex2(a); b = ex2(b);
+    if (poly) exp2_poly2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
+    else { upk2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b); a = ex2(a); b = ex2(b); }
     l1 = add2(l1, pk2(a, b));
     e[4 * i + 2] = __float_as_uint(a); e[4 * i + 3] = __float_as_uint(b);
   }
