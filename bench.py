@@ -74,8 +74,8 @@ def algorithmic(shape, L):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE score-kernel launch from the committed `ncu --set full`
-# capture (profiles/r1_v5b_ncu_cfg2.md), keyed by (workload, resident layers); None where no capture exists.
-NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40): 257.7e6 + 5.1e6}
+# capture (profiles/r1_final_ncu_cfg2.md), keyed by (workload, resident layers); None where no capture exists.
+NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40): 257.7e6 + 6.7e6}
 
 
 def _peaks():
@@ -310,7 +310,7 @@ def run_gpu(args):
         "roofline": {"kernel": "score (a1)", "bound": "tensor", "achieved": achieved_tflops,
                      "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": achieved_tflops / peaks["bf16_tflops"],
                      "traffic": NCU_SCORE_TRAFFIC_BYTES.get((args.workload, L)),
-                     "traffic_source": "profiles/r1_v5b_ncu_cfg2.md (ncu --set full, dram rd+wr of one launch)",
+                     "traffic_source": "profiles/r1_final_ncu_cfg2.md (ncu --set full, dram rd+wr of one launch)",
                      "peak_source": peaks["source"] + ", burst bf16", "kernel_ms": sc_ms,
                      "flops_per_launch": alg["flops"], "share_of_step": sc_ms / ms_per_step},
         "step_roofline": {"t_tensor_ms": t_tensor_ms, "t_hbm_ms": t_hbm_ms,
