@@ -292,3 +292,28 @@ def test_cfg2_full_size_sampled_units(gpu, oracle):
             assert check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 hard mismatch at unit {(l, hk)}"
             n_amb += 1
     assert n_amb <= len(sample)
+
+
+def test_scores_are_bit_reproducible_run_to_run(gpu):
+    """No atomics anywhere on the score path: lanes, quadrants, cluster ranks and tile ranges are all combined in a
+    fixed order, so two runs of the same call give the same bits — scores, index sets and every pool byte
+    (SURVEY hard part 3: near-ties at the top-k boundary must not flip between runs)."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG3, n_seqs=5, n_layers=3, hist_lo=64, hist_hi=700), seed=77)
+    a, ca, _ = gu.gpu_compress(wl)
+    b, cb, _ = gu.gpu_compress(wl)
+    assert ca.last_score_path() == 2 and cb.last_score_path() == 2
+    for key in ("scores", "idx_topk", "idx_final", "k", "v", "bt", "sl", "fc"):
+        np.testing.assert_array_equal(a[key].view(np.uint32) if a[key].dtype == np.float32 else a[key],
+                                      b[key].view(np.uint32) if b[key].dtype == np.float32 else b[key], err_msg=key)
+
+
+@pytest.mark.parametrize("W,U,d,G,bs,hist", [(96, 16, 64, 2, 16, 37), (200, 8, 128, 3, 16, 5), (272, 0, 128, 5, 32, 1000),
+                                              (320, 32, 64, 8, 64, 123), (528, 16, 128, 1, 16, 250)])
+def test_odd_shapes_against_the_oracle(gpu, chk, W, U, d, G, bs, hist):
+    """Window lengths that are no multiple of the 128-row tile or the 64-column chunk, every GQA group size, block
+    sizes 16/32/64, empty buffer, windows that start anywhere in a block: full three-stage parity."""
+    shape = kin.scaled(kin.CFG1, n_seqs=3, n_layers=2, n_q_heads=2 * G, n_kv_heads=2, head_dim=d, block_size=bs,
+                       W=W, U=U, alpha=8, gamma=6, hist_lo=hist, hist_hi=hist + 3 * bs, planted_positions=4)
+    stats, _, _ = _parity(gpu, chk, kin.generate(shape, seed=W + U))
+    assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
