@@ -63,6 +63,8 @@ extern "C" {
 #define KARA_KEEP_DEBUG 2u       /* keep scores / I / F of every unit in the workspace for kara_gather_debug */
 #define KARA_SCORE_QBUF_ONLY 4u  /* ablation "w/o Bi-Attention": queries = buffer U only */
 #define KARA_SCORE_SIMT 8u       /* force the CUDA-core score kernel (debug cross-check of the tcgen05 path) */
+#define KARA_SCORE_TWO_PHASE 16u /* tcgen05 score kernel, two-phase variant (S computed twice, no TMEM write-back;
+                                    same results within the score tolerance; csrc/score_tc2.cu) */
 
 /* `what` of kara_gather_debug */
 #define KARA_DBG_K_LOGICAL 0  /* bf16 [seq_len][d] rows of (layer, seq, kv_head) read through the block table */
@@ -151,7 +153,8 @@ int kara_status(kara_cache* c, int32_t* status_out /*host*/);
 /* Number of kernel launches the last kara_compress_window call made (for bench.py's gpu_launches). */
 int kara_last_launch_count(const kara_cache* c);
 
-/* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA. */
+/* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA,
+   3 = tcgen05/TMA two-phase variant (KARA_SCORE_TWO_PHASE). */
 int kara_last_score_path(const kara_cache* c);
 
 /* Device time of the score kernel (a1) alone: when enabled, every kara_compress_window call

@@ -255,10 +255,16 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   }
   if (use_tc) {
     int nl = 0;
-    rc = score_tc_launch(&c->tc, k, st, &nl);   // sets k.part_T / part_nc / part_tpu
-    if (rc != KARA_OK) return fail(rc, "score_tc_launch: %s", score_tc_error());
+    if (flags & KARA_SCORE_TWO_PHASE) {
+      rc = score_tc2_launch(&c->tc, k, st, &nl);   // sets k.part_T / part_nc / part_tpu
+      if (rc != KARA_OK) return fail(rc, "score_tc2_launch: %s", score_tc2_error());
+      c->last_score_path = 3;
+    } else {
+      rc = score_tc_launch(&c->tc, k, st, &nl);    // sets k.part_T / part_nc / part_tpu
+      if (rc != KARA_OK) return fail(rc, "score_tc_launch: %s", score_tc_error());
+      c->last_score_path = 2;
+    }
     launches += nl;
-    c->last_score_path = 2;
   } else {
     const int rows = (W - k.q_row_begin) * k.G;
     const int want = (rows + 127) / 128;

@@ -1,58 +1,43 @@
-// score_tc.cu — a1 (Eq. 4): A = colsum(softmax(Q_W K_{W\\U}^T / sqrt(d))) on the
-// 5th-generation tensor cores of sm_100a: TMA -> shared memory, tcgen05.mma -> TMEM, softmax out
-// of TMEM, deterministic column sums.  DESIGN.md §Kernels/a1 has the derivation of every choice.
+// score_tc2.cu — a1 (Eq. 4), TWO-PHASE variant of the tcgen05 score kernel (KARA_SCORE_TWO_PHASE).
 //
-// Decomposition.  A unit is one (layer, sequence, KV head).  A query tile is 128 window tokens x
-// ONE query head of the GQA group (rows of a row-softmax are independent, so any (token, head) ->
-// row map is valid; TMA reads the rows at stride n_q_heads*d).  All T = units * tiles_per_unit
-// tiles of the launch form one sequence that is cut into n_clusters contiguous, equally long
-// ranges (perfect balance; a range crosses unit boundaries, the part of a unit inside a range is
-// a "segment").  A thread-block cluster of CL CTAs owns a range; CTA r of the cluster owns the
-// 256 key rows [256 r, 256 r + 256) of the block-aligned key panel (whole paged blocks are
-// loaded, one TMA box per block and 64-element column panel; rows outside the compressible
-// region [h, h+n) are masked to -inf).  Per tile and CTA:
-//   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM,
-//       issued as two N <= 128 halves, each with its own full / empty barrier, so a half is
-//       refilled as soon as its column sums have been taken.
-//   The softmax is split over SPECIALISED warps (the v2 kernel ran both passes in the same warps
-//   and was bound by the latency of its own dependency chain, 2 warps per sub-partition):
-//   B warps (16: TMEM lane quadrant q x 64-column chunk cq) — pass B, the only MUFU work.  One TMEM
-//       read, one write: a thread holds 2 rows x 16 columns per piece (two pieces per tile); it shifts
-//       by ITS OWN maximum of those 16 logits, rounded to an integer z (log2 domain):
-//       e = exp2(s c - z), written back in place; l += e.  No separate max pass, no shuffles inside
-//       the pass.  Per tile a 6-shuffle reduce-scatter merges (z, l) over the 4 lanes of a row; shifts
-//       per (thread, row, chunk) (int16) and (z, l) per (row, chunk) go to shared memory; B warps
-//       never wait for anything but the next S half.
-//   C warps (4: one per lane quadrant) — statistics and pass C.  (z, l) of a row are merged over
-//       the four chunks and the CL CTAs with exact power-of-two rescaling built by integer
-//       arithmetic (no MUFU); across CTAs with st.async + a transaction-count mbarrier per
-//       (buffer, quadrant) — no fence, no cluster barrier.  w_(row,chunk) = 2^(z - Z_row) / L_row.
-//       pass C (one TMEM read):  acc_j += sum_i e_ij w_i  in per-thread registers: with the 16x256b
-//       TMEM load shape the column sum over ALL tiles of a segment is a plain packed FFMA2;
-//       lanes are combined once per segment.
-// TMEM holds two 128 x 256 fp32 S buffers (all 512 columns).  The K panel is double-buffered so a
-// segment change costs no bubble.  score_tc2.cu is the two-phase variant of this kernel.
+// Same decomposition as score_tc.cu (units, 128-row query tiles of one query head, one contiguous range of
+// tiles per cluster, CTA r owns key rows [256 r, 256 r + 256) of the block-aligned key panel), same TMA /
+// tcgen05 plumbing, same statistics conventions.  What differs is how the two passes over S are made.
+// score_tc.cu writes e = 2^(s c - z) back to TMEM and reads it again for the normalised column sums, which
+// ties pass B, the statistics, pass C and the refill of the TMEM buffer into one latency ring.  Here S is
+// COMPUTED TWICE instead (the tensor pipe is a quarter busy):
+//   phase 1  MMA1 -> TMEM region A.  8 warps read S once and keep only the row statistics (z, l); all
+//            exponentials of this phase run on the FMA pipe (degree-3 exp2, error 7.5e-5, which scales a
+//            whole row); nothing is written back, the region is released as soon as the loads have landed.
+//   S warps  (z, l) of a row over the two halves and the CL CTAs (st.async exchange), then
+//            o = Z + log2 L per row to shared memory.
+//   phase 2  one tile behind: MMA2 -> TMEM region B recomputes S; 8 warps read it once and add
+//            2^(s c - o) — the softmax probability itself, one MUFU ex2 per element — straight into the
+//            per-thread column sums.  No TMEM store, no second read, no dependency of the refill on phase 2's
+//            arithmetic.
+// Q tiles live in a 3-stage ring (a tile serves MMA1 and, one step later, MMA2); one K panel per segment.
+// Measured (round 1, cfg2): correct (score error 0.8 % of the tolerance) but 362 us against 200 us of
+// score_tc.cu: phase 1 costs 8 FMA-lane operations per element, i.e. 2,048 cycles per tile on the FMA pipe —
+// as much as phase 2 on the MUFU pipe — and its unrolled code misses the instruction cache (24 % of its
+// stalls).  Kept selectable as the base of the next round's work.
 //
-// Warp roles (768 threads): warps 0-15 B (q = warp & 3, cq = warp >> 2), 16-19 C (q = warp & 3),
-// 20 TMA producer, 21 MMA issuer, 22-23 idle (they complete the warpgroup whose registers
-// setmaxnreg hands to the C warps).
-// Output: partial[unit][p][j] (fp32), p = index of the range among those that touch the unit;
-// the select kernel sums the strips in fixed order, so scores are bit-reproducible run to run
-// (no atomics anywhere).
+// Warp roles (768 threads): warps 0-7 phase 1 (q = warp & 3, hf = warp >> 2), 8-15 phase 2 (same map),
+// 16-19 statistics (q = warp & 3), 20 TMA producer, 21 MMA issuer, 22-23 idle.
+// Output: partial[unit][p][j] (fp32) as in score_tc.cu; bit-reproducible run to run (no atomics).
 #include "score_tc_ptx.cuh"
 
 namespace kara {
 
 namespace {
 
-constexpr int kBWarps = 16;                   // pass B warps: 0..15
-constexpr int kCWarp0 = 16;                   // pass C warps: 16..19
+constexpr int kP2Warp0 = 8;                   // phase-1 warps: 0..7, phase-2 warps: 8..15
+constexpr int kSWarp0 = 16;                   // statistics warps: 16..19
 constexpr int kProducerWarp = 20;
 constexpr int kMmaWarp = 21;
 constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works per warpgroup); warps 22, 23 idle
 // registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
-// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, idle) = 6 x 80
-constexpr int kRegsB = 72, kRegsC = 152, kRegsOther = 40;
+// 2 x 88 (phase 1) + 2 x 112 (phase 2) + 40 (S) + 40 (producer, MMA, idle) <= 6 x 80
+constexpr int kRegsP1 = 88, kRegsP2 = 112, kRegsOther = 40;
 char g_tc_err[256] = "";
 
 // ------------------------------------------------------------------------------------------------
@@ -61,19 +46,19 @@ char g_tc_err[256] = "";
 template <int D, int CL>
 struct Smem {
   static constexpr int kPanels = D / 64;
-  static constexpr int kKStages = CL >= 8 ? 1 : 2;   // 8-CTA clusters need the room for the exchange slots
-  static constexpr int kQStages = 2;
+  static constexpr int kKStages = 1;                 // (the producer code is written for 1 or 2)
+  static constexpr int kQStages = 3;                 // Q(t) serves MMA1(t) and, one step later, MMA2(t)
   static constexpr int kKBytes = kPanels * kKeysPerCta * 128;
   static constexpr int kQStageBytes = kPanels * kTileM * 128;
-  static constexpr int kOffK = 0;
-  static constexpr int kOffQ = kOffK + kKStages * kKBytes;
-  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 C warps][256]
-  static constexpr int kOffZc = kOffColsum + 4 * kKeysPerCta * 4;        // short [2 bufs][4 q][4 chunks][4 rows][32 lanes] (unbiased shifts)
-  static constexpr int kOffRstat = kOffZc + 2 * 4 * 4 * 4 * 32 * 2;      // uint2 [2 bufs][4 chunks][128 rows]
-  static constexpr int kOffXch = kOffRstat + 2 * 4 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
+  static constexpr int kOffK = 0;                    // one K panel (both phases of a segment read it)
+  static constexpr int kOffQ = kOffK + kKBytes;
+  static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 quadrants][256]
+  static constexpr int kOffOrow = kOffColsum + 4 * kKeysPerCta * 4;      // float [2 slots][4 q][32 rows]: Z + log2 L of the row
+  static constexpr int kOffRstat = kOffOrow + 2 * 4 * 32 * 4;            // uint2 [2 slots][2 halves][128 rows]
+  static constexpr int kOffXch = kOffRstat + 2 * 2 * 128 * 8;            // uint2 [2 slots][4 q][CL][32]
   static constexpr int kOffBars = kOffXch + 2 * 4 * CL * 32 * 8;
-  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] = 26 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 26 * 8;
+  // barriers: qfull[3] qempty[3] kfull kempty tfull1[2] tempty1[2] tfull2[2] tempty2[2] bdone1[2] xbar[2][4] zready[2][4] = 34 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 34 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
@@ -116,17 +101,16 @@ __device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long 
 // columns the MMA of half hf produces (0 = half not issued)
 __device__ __forceinline__ int half_cols(int n_cols, int hf) { return min(max(n_cols - kHalf * hf, 0), kHalf); }
 
-// ---- pass B on one piece: 2 rows (K0, K0+1) x 16 columns of chunk CH (of this half) -----------------
-// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column col0 + 8 i + 2 qd + j of the CTA's 256; e gets the
-// exponentials in the same layout.  Online softmax with exact power-of-two rescaling: the shift of
-// this (row, chunk) is the running maximum z = max(z_run, round(m c)) of the thread's integer shifts
-// (log2 domain), so e <= 2^0.5; l_run is rescaled by 2^(z_old - z) built from the exponent field (no
-// MUFU).  Shifts are biased ints (see kZFloor); a fully masked piece has m = -inf -> as_int(t) < 0
-// -> z = floor / z_run, e = 0.
-template <int CH, int K0, bool RAGGED>
-__device__ __forceinline__ void pass_b_body(const uint32_t (&rin)[32], uint32_t (&e)[32], int (&zc)[2][4],
-                                            int (&zrun)[4], float (&lrun)[4], float cs, int qd, int col0,
-                                            int c_lo, int c_hi) {
+// ---- phase 1 on one piece: 2 rows (K0, K0+1) x 16 columns of a 64-column chunk --------------------------
+// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column col0 + 8 i + 2 qd + j of the CTA's 256.  Only the row
+// statistics are wanted: running (z, l) per row with exact power-of-two rescaling — the shift of the piece
+// is z = max(z_run, round(m c)), an integer in the log2 domain carried as a biased int (see kZFloor), so
+// e <= 2^0.5 and l_run is rescaled by 2^(z_old - z) built from the exponent field.  All exponentials of this
+// phase run on the FMA pipe (exp2_poly2): the MUFU pipe belongs to phase 2.  A masked column has
+// x = -inf -> clamped to 2^-125, which vanishes in l.
+template <bool FIRST, int K0, bool RAGGED>
+__device__ __forceinline__ void stats_body(const uint32_t (&rin)[32], int (&zrun)[4], float (&lrun)[4], float cs,
+                                           int qd, int col0, int c_lo, int c_hi) {
   float x[32];
 #pragma unroll
   for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(rin[i]);
@@ -153,7 +137,7 @@ __device__ __forceinline__ void pass_b_body(const uint32_t (&rin)[32], uint32_t 
   const float t1 = fminf(fmaf(m1, cs, kMagic), kMagic + kZLim);
   int z0, z1;
   float l0s, l1s;
-  if (CH == 0) {                                 // first chunk of the tile: nothing accumulated yet
+  if (FIRST) {                                   // first chunk of the tile: nothing accumulated yet
     z0 = max(kZFloor, __float_as_int(t0)); z1 = max(kZFloor, __float_as_int(t1));
     l0s = 0.f; l1s = 0.f;
   } else {
@@ -161,50 +145,42 @@ __device__ __forceinline__ void pass_b_body(const uint32_t (&rin)[32], uint32_t 
     l0s = lrun[K0] * pow2i(zrun[K0] - z0); l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
   }
   zrun[K0] = z0; zrun[K0 + 1] = z1;
-  zc[CH][K0] = z0; zc[CH][K0 + 1] = z1;
   const float nz0 = kMagic - __int_as_float(z0), nz1 = kMagic - __int_as_float(z1);   // = -z, exact
   const uint64_t cs2 = pk2(cs, cs), nz0_2 = pk2(nz0, nz0), nz1_2 = pk2(nz1, nz1);
   uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    // kPolyMask: column groups whose exponentials run on the FMA pipe (never on a ragged chunk,
-    // where masked columns must come out as exact zeros)
-    const bool poly = !RAGGED && ((kPolyMask >> i) & 1);
     float a, b;
-    if (poly) exp2_poly2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
-    else { upk2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b); a = ex2(a); b = ex2(b); }
+    exp2_poly2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
     l0 = add2(l0, pk2(a, b));
-    e[4 * i] = __float_as_uint(a); e[4 * i + 1] = __float_as_uint(b);
-    if (poly) exp2_poly2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
-    else { upk2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b); a = ex2(a); b = ex2(b); }
+    exp2_poly2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
     l1 = add2(l1, pk2(a, b));
-    e[4 * i + 2] = __float_as_uint(a); e[4 * i + 3] = __float_as_uint(b);
   }
   float a, b;
   upk2(l0, a, b); lrun[K0] = a + b;
   upk2(l1, a, b); lrun[K0 + 1] = a + b;
 }
-// two copies of the body, so that the common (no ragged edge) path carries no select and no register copies
-template <int CH, int K0>
-__device__ __forceinline__ void pass_b_piece(const uint32_t (&rin)[32], uint32_t (&e)[32], int (&zc)[2][4],
-                                             int (&zrun)[4], float (&lrun)[4], float cs, int qd, int col0,
-                                             int c_lo, int c_hi) {
+// two copies of the body, so that the common (no ragged edge) path carries no selects
+template <bool FIRST, int K0>
+__device__ __forceinline__ void stats_piece(const uint32_t (&rin)[32], int (&zrun)[4], float (&lrun)[4], float cs,
+                                            int qd, int col0, int c_lo, int c_hi) {
   if (col0 >= c_lo && col0 + 64 <= c_hi)        // warp-uniform: false only on the ragged first / last chunk
-    pass_b_body<CH, K0, false>(rin, e, zc, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+    stats_body<FIRST, K0, false>(rin, zrun, lrun, cs, qd, col0, c_lo, c_hi);
   else
-    pass_b_body<CH, K0, true>(rin, e, zc, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+    stats_body<FIRST, K0, true>(rin, zrun, lrun, cs, qd, col0, c_lo, c_hi);
 }
 
-// ---- pass C on one piece: acc[C*8 + i] (columns 64 C + 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------
-template <int C, int K0>
-__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[32], const float (&w)[4][4]) {
-  const uint64_t w0 = pk2(w[C][K0], w[C][K0]), w1 = pk2(w[C][K0 + 1], w[C][K0 + 1]);
+// ---- phase 2 on one piece: acc[i] (columns 8i+2qd+{0,1} of the chunk) += 2^(s c - o_row) for its 2 rows;
+//      o_row = Z + log2 L of the row (phase 1), so the terms are the softmax probabilities themselves ----
+__device__ __forceinline__ void score_piece(const uint32_t (&r)[32], uint64_t (&acc)[8], float cs, float oa, float ob) {
+  const uint64_t cs2 = pk2(cs, cs), na = pk2(-oa, -oa), nb = pk2(-ob, -ob);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    uint64_t a = acc[C * 8 + i];
-    a = fma2(pk2u(r[4 * i], r[4 * i + 1]), w0, a);
-    a = fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), w1, a);
-    acc[C * 8 + i] = a;
+    float a0, a1, b0, b1;
+    upk2(fma2(pk2u(r[4 * i], r[4 * i + 1]), cs2, na), a0, a1);
+    upk2(fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), cs2, nb), b0, b1);
+    a0 = ex2(a0); a1 = ex2(a1); b0 = ex2(b0); b1 = ex2(b1);
+    acc[i] = add2(add2(acc[i], pk2(a0, a1)), pk2(b0, b1));
   }
 }
 
@@ -213,7 +189,7 @@ __device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (
 // ------------------------------------------------------------------------------------------------
 template <int D, int CL>
 __global__ void __launch_bounds__(kThreads, 1)
-score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant__ CUtensorMap q_map,
+score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant__ CUtensorMap q_map,
                 const Call c, int T, int tpu, int tok_tiles) {
   using SM = Smem<D, CL>;
   constexpr int QS = SM::kQStages;
@@ -224,12 +200,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t sK = base + SM::kOffK;
   const uint32_t sQ = base + SM::kOffQ;
   float* colsum = reinterpret_cast<float*>(gbase + SM::kOffColsum);
-  short* zcs = reinterpret_cast<short*>(gbase + SM::kOffZc);
+  float* orow = reinterpret_cast<float*>(gbase + SM::kOffOrow);
   uint2* rstat = reinterpret_cast<uint2*>(gbase + SM::kOffRstat);
   uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
-  const uint32_t qfull = bars, qempty = bars + 16, kfull = bars + 32, kempty = bars + 48;
-  const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144;
+  const uint32_t qfull = bars, qempty = bars + 24, kfull = bars + 48, kempty = bars + 56;
+  const uint32_t tfull1 = bars + 64, tempty1 = bars + 80, tfull2 = bars + 96, tempty2 = bars + 112;
+  const uint32_t bdone1 = bars + 128, xbar = bars + 144, zready = bars + 208;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -239,13 +216,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const long long g_end = (long long)(cluster_id + 1) * T / n_clusters;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < 2; ++i) { mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(kfull + 8 * i, 1); mbar_init(kempty + 8 * i, 1); }
-    for (int i = 0; i < 4; ++i) {
-      mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 4);   // one arrive per C warp
+    for (int i = 0; i < 3; ++i) { mbar_init(qfull + 8 * i, 1); mbar_init(qempty + 8 * i, 1); }
+    mbar_init(kfull, 1); mbar_init(kempty, 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(tfull1 + 8 * i, 1); mbar_init(tempty1 + 8 * i, 4);   // one arrive per phase-1 warp of the half
+      mbar_init(tfull2 + 8 * i, 1); mbar_init(tempty2 + 8 * i, 4);   // one arrive per phase-2 warp of the half
+      mbar_init(bdone1 + 8 * i, 8);                                  // one arrive per phase-1 warp
     }
-    for (int i = 0; i < 2; ++i) mbar_init(bdone + 8 * i, kBWarps);  // one arrive per B warp
-    for (int i = 0; i < 8; ++i) mbar_init(xbar + 8 * i, 1);        // per (buffer, quadrant)
+    for (int i = 0; i < 8; ++i) { mbar_init(xbar + 8 * i, 1); mbar_init(zready + 8 * i, 1); }   // per (slot, quadrant)
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
@@ -330,95 +308,110 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     }
   } else if (warp == kMmaWarp) {
     // ================================ MMA issuer ================================================
-    // The whole warp walks the segments (warp-uniform values stay in uniform registers); one
-    // elected lane issues.  Descriptor low words are base + compile-time offsets: shared-memory
-    // addresses are < 2^18, so (addr >> 4) never carries out of the 14-bit address field.
+    // Two streams over the same tiles: MMA1(t) fills TMEM region A (columns 0..255) for phase 1, MMA2(t)
+    // fills region B (columns 256..511) for phase 2 and runs one tile behind (phase 2 needs the row
+    // statistics of the whole tile).  Each is issued as two N <= 128 halves with their own barriers.
+    // The whole warp walks the segments; one elected lane issues.  Descriptor low words are base +
+    // compile-time offsets: shared-memory addresses are < 2^18, so (addr >> 4) never carries out of
+    // the 14-bit address field.
     constexpr uint32_t kDescHi = (uint32_t)(1024u >> 4) | (1u << 14) | (2u << 29);   // SBO | version | SWIZZLE_128B
     constexpr uint32_t kDescLo = 1u << 16;                                           // LBO (unused)
-    int q_iter = 0, k_iter = 0, tile_iter = 0;
-    for (long long g = g_begin; g < g_end;) {
-      int n_tiles, n_cols;
-      {
-        const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
-        n_tiles = it.t1 - it.t0;
-        n_cols = it.ok ? it.n_cols : 0;
+    const uint32_t b_lo = (sK >> 4) | kDescLo;
+    struct Cur { long long g; int rem, n_cols; bool fresh; };
+    auto advance = [&](Cur& u) {
+      while (u.rem == 0 && u.g < g_end) {
+        const Seg it = decode_seg(c, u.g, g_end, rank, cluster_id, n_clusters, T, tpu);
+        u.g += it.t1 - it.t0;
+        if (it.ok) { u.rem = it.t1 - it.t0; u.n_cols = it.n_cols; u.fresh = true; }
       }
-      g += n_tiles;
-      if (n_cols == 0) continue;
-      const int kstage = k_iter % SM::kKStages, kuse = k_iter / SM::kKStages;
-      ++k_iter;
-      mbar_wait(kfull + 8 * kstage, kuse & 1);
-      const uint32_t b_lo = ((sK + kstage * SM::kKBytes) >> 4) | kDescLo;
-      for (int i = 0; i < n_tiles; ++i, ++q_iter, ++tile_iter) {
-        const int stage = q_iter % QS, quse = q_iter / QS;
-        const int buf = tile_iter & 1, tuse = tile_iter >> 1;
-        mbar_wait(qfull + 8 * stage, quse & 1);
+    };
+    auto issue = [&](uint32_t a_lo, uint32_t d_tmem, int nc, int hf) {
+      const uint32_t idesc = make_idesc_bf16(nc);
+#pragma unroll
+      for (int p = 0; p < SM::kPanels; ++p) {
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+          const uint64_t ad = ((uint64_t)kDescHi << 32) | (a_lo + ((p * (kTileM * 128) + ks * 32) >> 4));
+          const uint64_t bd = ((uint64_t)kDescHi << 32) |
+                              (b_lo + ((p * (kKeysPerCta * 128) + hf * (kHalf * 128) + ks * 32) >> 4));
+          umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
+        }
+      }
+    };
+    Cur c1{g_begin, 0, 0, false}, c2{g_begin, 0, 0, false};
+    int i1 = 0, i2 = 0, kuse = 0;
+    for (;;) {
+      bool did = false;
+      if (i2 < i1) {
+        // ---- MMA2 of tile i2 (its Q stage and K panel are still resident) ----
+        advance(c2);
+        const int stage = i2 % QS;
         const uint32_t a_lo = ((sQ + stage * SM::kQStageBytes) >> 4) | kDescLo;
 #pragma unroll
         for (int hf = 0; hf < 2; ++hf) {
-          mbar_wait(tempty + 8 * (buf * 2 + hf), (tuse & 1) ^ 1);
+          mbar_wait(tempty2 + 8 * hf, (i2 & 1) ^ 1);
           tc_fence_after();
           if (elect_one()) {
-            const int nc = half_cols(n_cols, hf);
-            if (nc > 0) {
-              const uint32_t idesc = make_idesc_bf16(nc);
-              const uint32_t d_tmem = tmem_base + buf * kKeysPerCta + hf * kHalf;
-#pragma unroll
-              for (int p = 0; p < SM::kPanels; ++p) {
-#pragma unroll
-                for (int ks = 0; ks < 4; ++ks) {
-                  const uint64_t ad = ((uint64_t)kDescHi << 32) | (a_lo + ((p * (kTileM * 128) + ks * 32) >> 4));
-                  const uint64_t bd = ((uint64_t)kDescHi << 32) |
-                                      (b_lo + ((p * (kKeysPerCta * 128) + hf * (kHalf * 128) + ks * 32) >> 4));
-                  umma_bf16(d_tmem, ad, bd, idesc, (p | ks) != 0);
-                }
-              }
-            }
-            umma_commit(tfull + 8 * (buf * 2 + hf));   // S half complete (fires at once if nothing was issued)
+            const int nc = half_cols(c2.n_cols, hf);
+            if (nc > 0) issue(a_lo, tmem_base + kKeysPerCta + hf * kHalf, nc, hf);
+            umma_commit(tfull2 + 8 * hf);
             if (hf == 1) {
-              umma_commit(qempty + 8 * stage);         // Q stage reusable once these MMAs have read it
-              if (i == n_tiles - 1) umma_commit(kempty + 8 * kstage);    // K stage reusable
+              umma_commit(qempty + 8 * stage);           // both phases have read this Q tile
+              if (c2.rem == 1) umma_commit(kempty);      // last tile of the segment: the K panel may be replaced
             }
           }
           __syncwarp();
         }
+        --c2.rem; ++i2; did = true;
       }
+      advance(c1);
+      if (c1.rem > 0) {
+        // ---- MMA1 of tile i1 ----
+        if (c1.fresh) { mbar_wait(kfull, kuse & 1); ++kuse; c1.fresh = false; }
+        const int stage = i1 % QS;
+        mbar_wait(qfull + 8 * stage, (i1 / QS) & 1);
+        const uint32_t a_lo = ((sQ + stage * SM::kQStageBytes) >> 4) | kDescLo;
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+          mbar_wait(tempty1 + 8 * hf, (i1 & 1) ^ 1);
+          tc_fence_after();
+          if (elect_one()) {
+            const int nc = half_cols(c1.n_cols, hf);
+            if (nc > 0) issue(a_lo, tmem_base + hf * kHalf, nc, hf);
+            umma_commit(tfull1 + 8 * hf);
+          }
+          __syncwarp();
+        }
+        --c1.rem; ++i1; did = true;
+      }
+      if (!did) break;
     }
   }
-  } else if (warp >= kCWarp0) {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsC));
-    // ================================ C warps: statistics + pass C ================================
-    const int q = warp & 3;                              // TMEM lane quadrant
-    const int qd = lane & 3, lr = lane >> 2;             // column pair within a group of 8; row within 8
-    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16);
-    uint64_t acc[32];
-#pragma unroll
-    for (int a = 0; a < 32; ++a) acc[a] = 0ull;
+  } else if (warp >= kSWarp0) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsOther));
+    // ================================ S warps: row statistics ======================================
+    // lane = row of this quadrant.  (z, l) of the two halves -> CTA -> cluster (st.async exchange), then
+    // o = Z + log2 L of the row to shared memory: phase 2 computes 2^(s c - o), the probability itself.
+    const int q = warp & 3;
     int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
-      float* out = c.partial + ((long long)it.unit * c.parts + it.part) * c.n_pad;
       if (!it.ok) {
         // skipped unit: its strip must still be defined (zeros); the status word says why
+        float* out = c.partial + ((long long)it.unit * c.parts + it.part) * c.n_pad;
         if (rank == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
         continue;
       }
-      const int n_chunks = (it.n_cols + 63) >> 6;                       // 1 .. 4
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        mbar_wait(bdone + 8 * b, par);
-        // ---- row statistics (lane = row of this quadrant): two halves -> CTA -> cluster ----
+        mbar_wait(bdone1 + 8 * b, par);
         int z_row;
         float l_row;
         {
-          uint2 sc[4];
-#pragma unroll
-          for (int ch = 0; ch < 4; ++ch) sc[ch] = rstat[(b * 4 + ch) * 128 + q * 32 + lane];
-          z_row = max(max((int)sc[0].x, (int)sc[1].x), max((int)sc[2].x, (int)sc[3].x));
-          l_row = 0.f;
-#pragma unroll
-          for (int ch = 0; ch < 4; ++ch) l_row += __uint_as_float(sc[ch].y) * pow2i((int)sc[ch].x - z_row);
+          const uint2 s0 = rstat[(b * 2 + 0) * 128 + q * 32 + lane], s1 = rstat[(b * 2 + 1) * 128 + q * 32 + lane];
+          z_row = max((int)s0.x, (int)s1.x);
+          l_row = __uint_as_float(s0.y) * pow2i((int)s0.x - z_row) + __uint_as_float(s1.y) * pow2i((int)s1.x - z_row);
         }
         if (CL > 1) {
           // lane publishes its row to every peer CTA ...
@@ -444,132 +437,69 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           z_row = Z; l_row = L;
         }
         const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + q * 32 + lane;
-        const float inv_row = (l_row > 0.f && tok < c.W) ? __fdividef(1.f, l_row) : 0.f;   // rows past the window contribute nothing
-        float w[4][4];
-        {
-          const short* zt = zcs + (size_t)((b * 4 + q) * 16) * 32 + lane;
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const int zf = __shfl_sync(0xffffffffu, z_row, lr + 8 * k) - kMagicBits;
-            const float iv = __shfl_sync(0xffffffffu, inv_row, lr + 8 * k);
-#pragma unroll
-            for (int ch = 0; ch < 4; ++ch)
-              w[ch][k] = ch < n_chunks ? iv * pow2i(zt[(ch * 4 + k) * 32] - zf) : 0.f;
-          }
-        }
-        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
-        tc_fence_after();
-        const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
-        uint32_t ra[32], rb[32];
-        tmem_ld_16x256b_x8(ta, ra);
-        tmem_wait_ld();
-        tmem_ld_16x256b_x8(ta_hi, rb);
-        pass_c_piece<0, 0>(ra, acc, w);
-        tmem_wait_ld();
-        if (n_chunks > 1) tmem_ld_16x256b_x8(ta + 64, ra);
-        pass_c_piece<0, 2>(rb, acc, w);
-        if (n_chunks > 1) {
-          tmem_wait_ld();
-          tmem_ld_16x256b_x8(ta_hi + 64, rb);
-          pass_c_piece<1, 0>(ra, acc, w);
-          tmem_wait_ld();
-          if (n_chunks > 2) tmem_ld_16x256b_x8(ta + 128, ra);
-          pass_c_piece<1, 2>(rb, acc, w);
-        }
-        // half 0 has been read completely: the MMA may refill it
-        tc_fence_before();
+        // rows past the window (and rows with no valid key) contribute nothing: 2^(s c - inf) = 0
+        const float o = (l_row > 0.f && tok < c.W) ? (float)(z_row - kMagicBits) + __log2f(l_row) : __int_as_float(0x7f800000);
+        orow[(b * 4 + q) * 32 + lane] = o;
         __syncwarp();
-        if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 0));
-        if (n_chunks > 2) {
-          tmem_wait_ld();
-          tmem_ld_16x256b_x8(ta_hi + 128, rb);
-          pass_c_piece<2, 0>(ra, acc, w);
-          tmem_wait_ld();
-          if (n_chunks > 3) tmem_ld_16x256b_x8(ta + 192, ra);
-          pass_c_piece<2, 2>(rb, acc, w);
-          if (n_chunks > 3) {
-            tmem_wait_ld();
-            tmem_ld_16x256b_x8(ta_hi + 192, rb);
-            pass_c_piece<3, 0>(ra, acc, w);
-            tmem_wait_ld();
-            pass_c_piece<3, 2>(rb, acc, w);
-          }
-        }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 1));
+        if (lane == 0) mbar_arrive(zready + 8 * (b * 4 + q));
       }
-
-      // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
-#pragma unroll
-      for (int a = 0; a < 32; ++a) {
-        float v0, v1;
-        upk2(acc[a], v0, v1);
-        v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
-        v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
-        v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
-        if (lr == 0)
-          *reinterpret_cast<float2*>(&colsum[q * kKeysPerCta + (a >> 3) * 64 + (a & 7) * 8 + 2 * qd]) = make_float2(v0, v1);
-        acc[a] = 0ull;
-      }
-      named_bar_sync(1, 128);
-#pragma unroll
-      for (int xx = 0; xx < 2; ++xx) {
-        const int x = (threadIdx.x & 127) + 128 * xx;
-        float v = 0.f;
-#pragma unroll
-        for (int wv = 0; wv < 4; ++wv) v += colsum[wv * kKeysPerCta + x];
-        if (x >= it.c_lo && x < it.c_hi) out[rank * kKeysPerCta + x - it.off] = v;
-      }
-      named_bar_sync(1, 128);
     }
-  } else {
-    // ================================ B warps: pass B ================================================
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsB));
-    const int q = warp & 3, cq = warp >> 2, hf = cq >> 1;   // TMEM lane quadrant; 64-column chunk; MMA half of the chunk
+  } else if (warp < kP2Warp0) {
+    // ================================ phase-1 warps: row statistics ====================================
+    // One TMEM read of S1, nothing written back: the half is handed back to the MMA warp as soon as this
+    // warp's loads have landed.  Exponentials on the FMA pipe (stats_piece).
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsP1));
+    const int q = warp & 3, hf = (warp >> 2) & 1;       // TMEM lane quadrant; column half
     const int qd = lane & 3, lr = lane >> 2;
     const float cs = kLog2e * rsqrtf((float)D);
-    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 64;
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + hf * kHalf, tq_hi = tq + (16u << 16);
+    auto release = [&]() {
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty1 + 8 * hf);
+    };
     int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
       if (!it.ok) continue;
-      const bool active = cq * 64 < it.n_cols;              // the MMA writes this chunk
+      const int n_ch = (half_cols(it.n_cols, hf) + 63) >> 6;            // chunks of this half the MMA writes: 0 .. 2
       const int c_lo = it.c_lo, c_hi = it.c_hi;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        int zc[2][4], zq[4];
+        const int b = tile_iter & 1;
+        int zq[4];
         float lq[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; zc[0][k] = kZFloor; }
-        mbar_wait(tfull + 8 * (b * 2 + hf), par);
+        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; }
+        mbar_wait(tfull1 + 8 * hf, tile_iter & 1);
         tc_fence_after();
-        if (active) {
-          // ---- pass B: e = 2^(s c - z) in place; z per (thread, row), (z, l) per row ----
-          const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
-          uint32_t ra[32], rb[32], e[32];
-          tmem_ld_16x256b_x8(ta, ra);
+        if (n_ch > 0) {
+          // one piece at a time: the registers go to keeping several polynomial chains in flight instead
+          uint32_t r[32];
+          tmem_ld_16x256b_x8(tq, r);
           tmem_wait_ld();
-          tmem_ld_16x256b_x8(ta_hi, rb);
-          pass_b_piece<0, 0>(ra, e, zc, zq, lq, cs, qd, cq * 64, c_lo, c_hi);
-          tmem_st_16x256b_x8(ta, e);
+          stats_piece<true, 0>(r, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
+          tmem_ld_16x256b_x8(tq_hi, r);
           tmem_wait_ld();
-          pass_b_piece<0, 2>(rb, e, zc, zq, lq, cs, qd, cq * 64, c_lo, c_hi);
-          tmem_st_16x256b_x8(ta_hi, e);
+          if (n_ch == 1) release();
+          stats_piece<true, 2>(r, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
+          if (n_ch > 1) {
+            tmem_ld_16x256b_x8(tq + 64, r);
+            tmem_wait_ld();
+            stats_piece<false, 0>(r, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
+            tmem_ld_16x256b_x8(tq_hi + 64, r);
+            tmem_wait_ld();
+            release();
+            stats_piece<false, 2>(r, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
+          }
+        } else {
+          release();
         }
-        // ---- row statistics of this chunk: quad -> row; shifts and (z, l) to shared memory ----
-        {
-          short* zt = zcs + (size_t)((b * 4 + q) * 16 + cq * 4) * 32 + lane;
-#pragma unroll
-          for (int k = 0; k < 4; ++k) zt[k * 32] = (short)(zc[0][k] - kMagicBits);
-        }
-        // reduce-scatter over the 4 lanes of a quad: lane qd ends up with row k = qd (6 shuffles)
+        // ---- reduce-scatter over the 4 lanes of a quad (6 shuffles): lane qd ends up with row k = qd ----
         int z_row;
         float l_row;
         {
           const bool p1 = qd & 1, p2 = qd & 2;
-          // step 1 (lane ^ 1): keep rows {p1, p1 + 2}, hand the other two over
           const int ks0 = p1 ? zq[1] : zq[0], ks1 = p1 ? zq[3] : zq[2];
           const float kl0 = p1 ? lq[1] : lq[0], kl1 = p1 ? lq[3] : lq[2];
           const int rz0 = __shfl_xor_sync(0xffffffffu, p1 ? zq[0] : zq[1], 1);
@@ -579,7 +509,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           const int za = max(ks0, rz0), zb = max(ks1, rz1);
           const float la = kl0 * pow2i(ks0 - za) + rl0 * pow2i(rz0 - za);
           const float lb = kl1 * pow2i(ks1 - zb) + rl1 * pow2i(rz1 - zb);
-          // step 2 (lane ^ 2): keep row p1 + 2 p2 = qd
           const int kz = p2 ? zb : za;
           const float kl = p2 ? lb : la;
           const int rz = __shfl_xor_sync(0xffffffffu, p2 ? za : zb, 2);
@@ -587,12 +516,88 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           z_row = max(kz, rz);
           l_row = kl * pow2i(kz - z_row) + rl * pow2i(rz - z_row);
         }
-        rstat[(b * 4 + cq) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
-        tmem_wait_st();
-        tc_fence_before();
+        rstat[(b * 2 + hf) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
         __syncwarp();
-        if (lane == 0) mbar_arrive(bdone + 8 * b);
+        if (lane == 0) mbar_arrive(bdone1 + 8 * b);
       }
+    }
+  } else {
+    // ================================ phase-2 warps: scores ===========================================
+    // One TMEM read of S2 (recomputed), one ex2 per element, straight into the per-thread column sums
+    // (with the 16x256b load shape the sum over rows needs no transpose); nothing goes back to TMEM.
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsP2));
+    const int q = warp & 3, hf = (warp >> 2) & 1;       // TMEM lane quadrant; column half
+    const int qd = lane & 3, lr = lane >> 2;
+    const float cs = kLog2e * rsqrtf((float)D);
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + kKeysPerCta + hf * kHalf, tq_hi = tq + (16u << 16);
+    uint64_t acc[2][8];                                 // column sums of this warp's two chunks over the segment
+#pragma unroll
+    for (int a = 0; a < 8; ++a) { acc[0][a] = 0ull; acc[1][a] = 0ull; }
+    auto release = [&]() {
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty2 + 8 * hf);
+    };
+    int tile_iter = 0;
+    for (long long g = g_begin; g < g_end;) {
+      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+      g += it.t1 - it.t0;
+      if (!it.ok) continue;
+      const int n_ch = (half_cols(it.n_cols, hf) + 63) >> 6;            // chunks of this half the MMA writes: 0 .. 2
+      float* out = c.partial + ((long long)it.unit * c.parts + it.part) * c.n_pad;
+      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
+        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
+        mbar_wait(zready + 8 * (b * 4 + q), par);
+        float o[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) o[k] = orow[(b * 4 + q) * 32 + lr + 8 * k];
+        mbar_wait(tfull2 + 8 * hf, tile_iter & 1);
+        tc_fence_after();
+        if (n_ch > 0) {
+          uint32_t ra[32], rb[32];
+          tmem_ld_16x256b_x8(tq, ra);
+          tmem_ld_16x256b_x8(tq_hi, rb);
+          tmem_wait_ld();
+          if (n_ch == 1) release();
+          score_piece(ra, acc[0], cs, o[0], o[1]);
+          if (n_ch > 1) tmem_ld_16x256b_x8(tq + 64, ra);
+          score_piece(rb, acc[0], cs, o[2], o[3]);
+          if (n_ch > 1) {
+            tmem_wait_ld();
+            tmem_ld_16x256b_x8(tq_hi + 64, rb);
+            score_piece(ra, acc[1], cs, o[0], o[1]);
+            tmem_wait_ld();
+            release();
+            score_piece(rb, acc[1], cs, o[2], o[3]);
+          }
+        } else {
+          release();
+        }
+      }
+      // ---- segment done: combine lanes (fixed order), then the 4 quadrants (fixed order), write the strip ----
+#pragma unroll
+      for (int ch = 0; ch < 2; ++ch) {
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+          float v0, v1;
+          upk2(acc[ch][a], v0, v1);
+          v0 += __shfl_xor_sync(0xffffffffu, v0, 4);  v1 += __shfl_xor_sync(0xffffffffu, v1, 4);
+          v0 += __shfl_xor_sync(0xffffffffu, v0, 8);  v1 += __shfl_xor_sync(0xffffffffu, v1, 8);
+          v0 += __shfl_xor_sync(0xffffffffu, v0, 16); v1 += __shfl_xor_sync(0xffffffffu, v1, 16);
+          if (lr == 0)
+            *reinterpret_cast<float2*>(&colsum[q * kKeysPerCta + hf * kHalf + ch * 64 + a * 8 + 2 * qd]) = make_float2(v0, v1);
+          acc[ch][a] = 0ull;
+        }
+      }
+      named_bar_sync(1 + hf, 128);                          // the 4 warps (quadrants) that share this half
+      {
+        const int x = hf * kHalf + q * 32 + lane;
+        float v = 0.f;
+#pragma unroll
+        for (int wv = 0; wv < 4; ++wv) v += colsum[wv * kKeysPerCta + x];
+        if (x >= it.c_lo && x < it.c_hi) out[rank * kKeysPerCta + x - it.off] = v;
+      }
+      named_bar_sync(1 + hf, 128);
     }
   }
 
@@ -636,7 +641,7 @@ int cluster_size_for(const Call& c) {
 template <int D, int CL>
 int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
   using SM = Smem<D, CL>;
-  auto kern = score_tc_kernel<D, CL>;
+  auto kern = score_tc2_kernel<D, CL>;
   static bool attr_done = false;
   if (!attr_done) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kAlloc) != cudaSuccess)
@@ -683,49 +688,9 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
 
 }  // namespace
 
-const char* score_tc_error() { return g_tc_err; }
+const char* score_tc2_error() { return g_tc_err; }
 
-int score_tc_attach(ScoreTcState* s, const Geom& g, void* k_pool) {
-  s->ready = false;
-  s->q_ptr = nullptr;
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return KARA_OK; }   // no device: SIMT path errors later
-  cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { cudaGetLastError(); return KARA_OK; }
-  s->num_sms = prop.multiProcessorCount;
-  if (prop.major != 10) return KARA_OK;                // not a tcgen05 part: SIMT kernel only
-  EncodeTiledFn enc = get_encode();
-  if (!enc) return tc_fail(KARA_ECUDA, "cuTensorMapEncodeTiled entry point not found");
-  const unsigned long long rows = (unsigned long long)g.n_layers * g.num_blocks * g.n_kv_heads * g.bs;
-  if (rows >= (1ull << 31)) return KARA_OK;            // beyond one tensor map's signed coordinates: SIMT path
-  cuuint64_t dims[2] = {(cuuint64_t)g.d, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {(cuuint64_t)g.d * 2};
-  cuuint32_t box[2] = {64u, (cuuint32_t)g.bs};
-  cuuint32_t estr[2] = {1u, 1u};
-  CUtensorMap m;
-  CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, k_pool, dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) {
-    snprintf(g_tc_err, sizeof g_tc_err, "cuTensorMapEncodeTiled(K pool) failed: CUresult %d", (int)r);
-    return KARA_ECUDA;
-  }
-  memcpy(s->k_map, &m, sizeof m);
-  s->ready = true;
-  return KARA_OK;
-}
-
-bool score_tc_supported(const ScoreTcState& s, const Call& c) {
-  if (!s.ready) return false;
-  if (c.g.d != 64 && c.g.d != 128) return false;
-  if (c.g.bs > kKeysPerCta) return false;
-  if (cluster_size_for(c) == 0) return false;
-  const unsigned long long toks = (unsigned long long)c.n_layers * c.n_seqs * c.W;
-  if (toks >= (1ull << 31)) return false;
-  return true;
-}
-
-int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) {
+int score_tc2_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) {
   // window_q tensor map: [d][n_q_heads][layers*seqs*W tokens], box 64 x 1 x 128, 128B swizzle
   const long long key[6] = {(long long)(uintptr_t)c.window_q, c.g.d, c.n_q_heads, (long long)c.n_layers * c.n_seqs * c.W, 0, 0};
   if (s->q_ptr != c.window_q || memcmp(key, s->q_key, sizeof key) != 0) {
@@ -758,4 +723,5 @@ int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) 
 }
 
 }  // namespace kara
+
 

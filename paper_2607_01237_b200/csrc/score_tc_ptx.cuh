@@ -1,0 +1,247 @@
+// score_tc_ptx.cuh — what the two tcgen05 score kernels (score_tc.cu, score_tc2.cu) share: tile constants, the
+// integer-shift conventions of the online softmax, and thin wrappers around the sm_100a PTX they use (mbarrier,
+// TMA, tcgen05 alloc / mma / commit / ld / st, cluster addressing, packed f32x2 arithmetic, the FMA-pipe exp2).
+// Everything is in an anonymous namespace: each translation unit gets its own copy.
+#pragma once
+#include <cuda.h>
+
+#include <cstdio>
+#include <cstring>
+
+#include "score_tc.h"
+
+namespace kara {
+
+namespace {
+
+constexpr int kTileM = 128;
+constexpr int kKeysPerCta = 256;              // key rows (S columns) of one CTA = one TMEM buffer
+constexpr int kHalf = 128;                    // columns of one MMA half
+constexpr int kTmemCols = 512;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kMagic = 12582912.f;          // 1.5 * 2^23: x + kMagic rounds x to an integer in the low mantissa bits
+constexpr int kMagicBits = 0x4B400000;
+// integer shifts z are carried as the bit pattern of (z + kMagic), i.e. biased by kMagicBits; they
+// are clamped to z <= kZLim (|logit| log2e / sqrt(d) beyond that is not served) and floored at
+// -kZLim, which is also the shift of a piece with no valid key (its l is 0)
+constexpr float kZLim = 32000.f;
+#ifndef KARA_POLY_MASK
+#define KARA_POLY_MASK 0x00                   // bit i: column group i of 8 uses the FMA-pipe polynomial (measured: 0x52 is 7 % slower)
+#endif
+constexpr unsigned kPolyMask = KARA_POLY_MASK;
+constexpr int kZFloor = kMagicBits - 32000;
+
+// ------------------------------------------------------------------------------------------------
+// PTX wrappers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+#ifdef KARA_TC_DEBUG
+// debug build: a wait that does not complete within ~2^26 polls reports who is stuck and traps
+__device__ __noinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  for (long long spin = 0;; ++spin) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+    if (spin > (1ll << 24)) {
+      printf("STUCK block %d warp %d lane %d bar_off %u parity %u\n", blockIdx.x, threadIdx.x >> 5, threadIdx.x & 31,
+             bar & 1023u, parity);
+      __trap();
+    }
+  }
+}
+#else
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "KARA_WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra KARA_DONE_%=;\n\t"
+      "bra KARA_WAIT_%=;\n\t"
+      "KARA_DONE_%=:\n\t}"
+      :: "r"(bar), "r"(parity) : "memory");
+}
+#endif
+// producer-side wait: polls with a pause, so the spinning warp does not take issue slots from the math warps
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  for (;;) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+    __nanosleep(64);
+  }
+}
+__device__ __forceinline__ uint32_t mapa(uint32_t local_addr, uint32_t cta) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta));
+  return r;
+}
+// 8-byte store into a peer CTA's shared memory that signals the peer's mbarrier (complete_tx)
+__device__ __forceinline__ void st_async_b32x2(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t cluster_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b32 [%0], {%1, %2}, [%3];"
+               :: "r"(cluster_addr), "r"(a), "r"(b), "r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
+  return p != 0;
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory");
+}
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      :: "r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      :: "r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(dst_smem), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(taddr), "r"(ncols) : "memory");
+}
+// D[tmem] (+)= A[smem desc] . B[smem desc]^T, bf16 x bf16 -> fp32
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      :: "r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+
+// K-major, 128-byte-swizzled operand tile: rows at 128 B pitch, 8-row groups at 1024 B (SBO),
+// descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B.  (cute/arch/mma_sm100_desc.hpp)
+__device__ __forceinline__ uint64_t make_sw128_desc(uint32_t smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr >> 4) & 0x3FFFu);       // start address, 16-byte units
+  d |= (uint64_t)1u << 16;                            // leading byte offset (unused for swizzled K-major)
+  d |= (uint64_t)(1024u >> 4) << 32;                  // stride byte offset: 8 rows x 128 B
+  d |= (uint64_t)1u << 46;                            // descriptor version (Blackwell)
+  d |= (uint64_t)2u << 61;                            // SWIZZLE_128B
+  return d;
+}
+// instruction descriptor: fp32 accumulate, bf16 A and B, both K-major, M = 128, N = n
+__device__ __forceinline__ uint32_t make_idesc_bf16(int n) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+}
+
+#define KARA_TMEM_REGS32(r)                                                                          \
+  "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),    \
+  "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]),           \
+  "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]),         \
+  "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]),         \
+  "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+#define KARA_TMEM_IN32(r)                                                                            \
+  "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),            \
+  "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),      \
+  "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),    \
+  "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+
+// 16 lanes x 64 columns: thread t gets, for column group i (8 columns), regs 4i+{0,1} = lane t/4,
+// columns 8i + 2(t%4) + {0,1}; regs 4i+{2,3} = lane t/4 + 8, same columns.
+__device__ __forceinline__ void tmem_ld_16x256b_x8(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.16x256b.x8.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : KARA_TMEM_REGS32(r) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st_16x256b_x8(uint32_t taddr, const uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.16x256b.x8.b32 [%32], "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
+      :: KARA_TMEM_IN32(r), "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float y;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
+  return y;
+}
+// packed fp32 pairs (FFMA2 / FADD2 on sm_100)
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ uint64_t pk2u(uint32_t lo, uint32_t hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+// 2^x for a pair of x <= 0.5 on the FMA pipe (the MUFU pipe, 16 ex2/clk/SM, is the scarcer resource
+// of pass B: one ex2 per 2 d tensor FLOPs): x = n + f, n = round(x) by the magic-number add, f in
+// [-0.5, 0.5]; 2^f by a degree-3 polynomial (relative minimax fit, max error 7.5e-5 in fp32 Horner,
+// far inside the 1e-3 score tolerance); 2^n by adding n to the exponent field.
+constexpr float kP0 = 0.9999281168f, kP1 = 0.6932609677f, kP2 = 0.2426105440f, kP3 = 0.0551713221f;
+__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& a, float& b) {
+  float xa, xb;
+  upk2(x2, xa, xb);
+  xa = fmaxf(xa, -125.f); xb = fmaxf(xb, -125.f);          // below fp32's normal range: 2^-125 stands in for 0
+  const uint64_t xc = pk2(xa, xb);
+  const uint64_t t2 = add2(xc, pk2(kMagic, kMagic));         // low mantissa bits = round(x)
+  const uint64_t n2 = add2(t2, pk2(-kMagic, -kMagic));       // round(x) as a float, exact
+  const uint64_t f2 = fma2(n2, pk2(-1.f, -1.f), xc);         // x - round(x), exact
+  uint64_t p2 = fma2(pk2(kP3, kP3), f2, pk2(kP2, kP2));
+  p2 = fma2(p2, f2, pk2(kP1, kP1));
+  p2 = fma2(p2, f2, pk2(kP0, kP0));
+  float pa, pb, ta, tb;
+  upk2(p2, pa, pb);
+  upk2(t2, ta, tb);
+  a = __int_as_float(__float_as_int(pa) + (__float_as_int(ta) << 23));
+  b = __int_as_float(__float_as_int(pb) + (__float_as_int(tb) << 23));
+}
+// 2^d for d <= 0 built from the exponent field; 0 for d <= -127 (such weights are below fp32's range)
+__device__ __forceinline__ float pow2i(int d) { return __int_as_float(max(d + 127, 0) << 23); }
+
+}  // namespace
+
+}  // namespace kara
