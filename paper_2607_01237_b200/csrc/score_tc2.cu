@@ -16,10 +16,10 @@
 //            per-thread column sums.  No TMEM store, no second read, no dependency of the refill on phase 2's
 //            arithmetic.
 // Q tiles live in a 3-stage ring (a tile serves MMA1 and, one step later, MMA2); one K panel per segment.
-// Measured (round 1, cfg2): correct (score error 0.8 % of the tolerance) but 362 us against 200 us of
+// Measured (round 1, cfg2): correct (score error 0.7 % of the tolerance) but 309 us against 200 us of
 // score_tc.cu: phase 1 costs 8 FMA-lane operations per element, i.e. 2,048 cycles per tile on the FMA pipe —
-// as much as phase 2 on the MUFU pipe — and its unrolled code misses the instruction cache (24 % of its
-// stalls).  Kept selectable as the base of the next round's work.
+// as much as phase 2 on the MUFU pipe — and about 1,000 issued instructions per tile and warp.  Kept
+// selectable as the base of the next round's work (DESIGN.md §10 has the measurements).
 //
 // Warp roles (768 threads): warps 0-7 phase 1 (q = warp & 3, hf = warp >> 2), 8-15 phase 2 (same map),
 // 16-19 statistics (q = warp & 3), 20 TMA producer, 21 MMA issuer, 22-23 idle.
@@ -38,6 +38,11 @@ constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works 
 // registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
 // 2 x 88 (phase 1) + 2 x 112 (phase 2) + 40 (S) + 40 (producer, MMA, idle) <= 6 x 80
 constexpr int kRegsP1 = 88, kRegsP2 = 112, kRegsOther = 40;
+constexpr int kSlots = 4;                     // statistics slots between phase 1, the S warps and phase 2
+#ifndef KARA_P1_MUFU_MASK
+#define KARA_P1_MUFU_MASK 0x22                // groups 1 and 5 of 8: a quarter of phase 1's exponentials on the MUFU pipe
+#endif
+constexpr unsigned kP1MufuMask = KARA_P1_MUFU_MASK;
 char g_tc_err[256] = "";
 
 // ------------------------------------------------------------------------------------------------
@@ -53,12 +58,14 @@ struct Smem {
   static constexpr int kOffK = 0;                    // one K panel (both phases of a segment read it)
   static constexpr int kOffQ = kOffK + kKBytes;
   static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 quadrants][256]
-  static constexpr int kOffOrow = kOffColsum + 4 * kKeysPerCta * 4;      // float [2 slots][4 q][32 rows]: Z + log2 L of the row
-  static constexpr int kOffRstat = kOffOrow + 2 * 4 * 32 * 4;            // uint2 [2 slots][2 halves][128 rows]
-  static constexpr int kOffXch = kOffRstat + 2 * 2 * 128 * 8;            // uint2 [2 slots][4 q][CL][32]
-  static constexpr int kOffBars = kOffXch + 2 * 4 * CL * 32 * 8;
-  // barriers: qfull[3] qempty[3] kfull kempty tfull1[2] tempty1[2] tfull2[2] tempty2[2] bdone1[2] xbar[2][4] zready[2][4] = 34 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 34 * 8;
+  // statistics slots: phase 1 may run up to kQStages - 1 = 2 tiles ahead of phase 2, so everything that is
+  // handed from phase 1 over the S warps to phase 2 lives in kSlots = 4 slots (tile & 3)
+  static constexpr int kOffOrow = kOffColsum + 4 * kKeysPerCta * 4;      // float [4 slots][4 q][32 rows]: Z + log2 L of the row
+  static constexpr int kOffRstat = kOffOrow + kSlots * 4 * 32 * 4;       // uint2 [4 slots][2 halves][128 rows]
+  static constexpr int kOffXch = kOffRstat + kSlots * 2 * 128 * 8;       // uint2 [4 slots][4 q][CL][32]
+  static constexpr int kOffBars = kOffXch + kSlots * 4 * CL * 32 * 8;
+  // barriers: qfull[3] qempty[3] kfull kempty tfull1[2] tempty1[2] tfull2[2] tempty2[2] bdone1[4] xbar[4][4] zready[4][4] = 52 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 52 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
@@ -108,7 +115,7 @@ __device__ __forceinline__ int half_cols(int n_cols, int hf) { return min(max(n_
 // e <= 2^0.5 and l_run is rescaled by 2^(z_old - z) built from the exponent field.  All exponentials of this
 // phase run on the FMA pipe (exp2_poly2): the MUFU pipe belongs to phase 2.  A masked column has
 // x = -inf -> clamped to 2^-125, which vanishes in l.
-template <bool FIRST, int K0, bool RAGGED>
+template <int K0, bool RAGGED>
 __device__ __forceinline__ void stats_body(const uint32_t (&rin)[32], int (&zrun)[4], float (&lrun)[4], float cs,
                                            int qd, int col0, int c_lo, int c_hi) {
   float x[32];
@@ -135,25 +142,22 @@ __device__ __forceinline__ void stats_body(const uint32_t (&rin)[32], int (&zrun
   // t = round(m c) + kMagic as a float; its bit pattern is the biased integer shift
   const float t0 = fminf(fmaf(m0, cs, kMagic), kMagic + kZLim);
   const float t1 = fminf(fmaf(m1, cs, kMagic), kMagic + kZLim);
-  int z0, z1;
-  float l0s, l1s;
-  if (FIRST) {                                   // first chunk of the tile: nothing accumulated yet
-    z0 = max(kZFloor, __float_as_int(t0)); z1 = max(kZFloor, __float_as_int(t1));
-    l0s = 0.f; l1s = 0.f;
-  } else {
-    z0 = max(zrun[K0], __float_as_int(t0)); z1 = max(zrun[K0 + 1], __float_as_int(t1));
-    l0s = lrun[K0] * pow2i(zrun[K0] - z0); l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
-  }
+  // (a tile starts at (z, l) = (floor, 0), for which this update is exact: one code path for every chunk)
+  const int z0 = max(zrun[K0], __float_as_int(t0)), z1 = max(zrun[K0 + 1], __float_as_int(t1));
+  const float l0s = lrun[K0] * pow2i(zrun[K0] - z0), l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
   zrun[K0] = z0; zrun[K0 + 1] = z1;
   const float nz0 = kMagic - __int_as_float(z0), nz1 = kMagic - __int_as_float(z1);   // = -z, exact
   const uint64_t cs2 = pk2(cs, cs), nz0_2 = pk2(nz0, nz0), nz1_2 = pk2(nz1, nz1);
   uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
+    // kP1MufuMask: column groups of phase 1 that use the MUFU pipe's spare share instead of the polynomial
     float a, b;
-    exp2_poly2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
+    if ((kP1MufuMask >> i) & 1) { upk2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b); a = ex2(a); b = ex2(b); }
+    else exp2_poly2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
     l0 = add2(l0, pk2(a, b));
-    exp2_poly2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
+    if ((kP1MufuMask >> i) & 1) { upk2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b); a = ex2(a); b = ex2(b); }
+    else exp2_poly2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
     l1 = add2(l1, pk2(a, b));
   }
   float a, b;
@@ -161,13 +165,13 @@ __device__ __forceinline__ void stats_body(const uint32_t (&rin)[32], int (&zrun
   upk2(l1, a, b); lrun[K0 + 1] = a + b;
 }
 // two copies of the body, so that the common (no ragged edge) path carries no selects
-template <bool FIRST, int K0>
+template <int K0>
 __device__ __forceinline__ void stats_piece(const uint32_t (&rin)[32], int (&zrun)[4], float (&lrun)[4], float cs,
                                             int qd, int col0, int c_lo, int c_hi) {
   if (col0 >= c_lo && col0 + 64 <= c_hi)        // warp-uniform: false only on the ragged first / last chunk
-    stats_body<FIRST, K0, false>(rin, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+    stats_body<K0, false>(rin, zrun, lrun, cs, qd, col0, c_lo, c_hi);
   else
-    stats_body<FIRST, K0, true>(rin, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+    stats_body<K0, true>(rin, zrun, lrun, cs, qd, col0, c_lo, c_hi);
 }
 
 // ---- phase 2 on one piece: acc[i] (columns 8i+2qd+{0,1} of the chunk) += 2^(s c - o_row) for its 2 rows;
@@ -206,7 +210,7 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
   const uint32_t bars = base + SM::kOffBars;
   const uint32_t qfull = bars, qempty = bars + 24, kfull = bars + 48, kempty = bars + 56;
   const uint32_t tfull1 = bars + 64, tempty1 = bars + 80, tfull2 = bars + 96, tempty2 = bars + 112;
-  const uint32_t bdone1 = bars + 128, xbar = bars + 144, zready = bars + 208;
+  const uint32_t bdone1 = bars + 128, xbar = bars + 160, zready = bars + 288;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -221,9 +225,9 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
     for (int i = 0; i < 2; ++i) {
       mbar_init(tfull1 + 8 * i, 1); mbar_init(tempty1 + 8 * i, 4);   // one arrive per phase-1 warp of the half
       mbar_init(tfull2 + 8 * i, 1); mbar_init(tempty2 + 8 * i, 4);   // one arrive per phase-2 warp of the half
-      mbar_init(bdone1 + 8 * i, 8);                                  // one arrive per phase-1 warp
     }
-    for (int i = 0; i < 8; ++i) { mbar_init(xbar + 8 * i, 1); mbar_init(zready + 8 * i, 1); }   // per (slot, quadrant)
+    for (int i = 0; i < kSlots; ++i) mbar_init(bdone1 + 8 * i, 8);   // one arrive per phase-1 warp
+    for (int i = 0; i < 4 * kSlots; ++i) { mbar_init(xbar + 8 * i, 1); mbar_init(zready + 8 * i, 1); }   // per (slot, quadrant)
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
@@ -340,9 +344,14 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
     };
     Cur c1{g_begin, 0, 0, false}, c2{g_begin, 0, 0, false};
     int i1 = 0, i2 = 0, kuse = 0;
+    // Whichever stream can go, goes (a strict MMA2, MMA1 alternation would couple the two phases: a late
+    // phase 2 would hold back MMA1 although region A is free).  Phase 1 runs at most QS - 1 tiles ahead
+    // (the Q ring); MMA2 has priority, which also keeps the single K panel moving at segment changes.
     for (;;) {
-      bool did = false;
-      if (i2 < i1) {
+      advance(c1);
+      const bool more1 = c1.rem > 0;
+      if (!more1 && i2 == i1) break;
+      if (i2 < i1 && mbar_test(tempty2, (i2 & 1) ^ 1)) {
         // ---- MMA2 of tile i2 (its Q stage and K panel are still resident) ----
         advance(c2);
         const int stage = i2 % QS;
@@ -362,10 +371,9 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
           }
           __syncwarp();
         }
-        --c2.rem; ++i2; did = true;
-      }
-      advance(c1);
-      if (c1.rem > 0) {
+        --c2.rem; ++i2;
+      } else if (more1 && i1 - i2 < QS && mbar_test(tempty1, (i1 & 1) ^ 1) &&
+                 (!c1.fresh || mbar_test(kfull, kuse & 1)) && mbar_test(qfull + 8 * (i1 % QS), (i1 / QS) & 1)) {
         // ---- MMA1 of tile i1 ----
         if (c1.fresh) { mbar_wait(kfull, kuse & 1); ++kuse; c1.fresh = false; }
         const int stage = i1 % QS;
@@ -382,9 +390,8 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
           }
           __syncwarp();
         }
-        --c1.rem; ++i1; did = true;
+        --c1.rem; ++i1;
       }
-      if (!did) break;
     }
   }
   } else if (warp >= kSWarp0) {
@@ -404,7 +411,7 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
         continue;
       }
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
+        const int b = tile_iter & (kSlots - 1), par = (tile_iter / kSlots) & 1;
         mbar_wait(bdone1 + 8 * b, par);
         int z_row;
         float l_row;
@@ -466,35 +473,27 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
       const int n_ch = (half_cols(it.n_cols, hf) + 63) >> 6;            // chunks of this half the MMA writes: 0 .. 2
       const int c_lo = it.c_lo, c_hi = it.c_hi;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        const int b = tile_iter & 1;
+        const int b = tile_iter & (kSlots - 1);
         int zq[4];
         float lq[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; }
         mbar_wait(tfull1 + 8 * hf, tile_iter & 1);
         tc_fence_after();
-        if (n_ch > 0) {
-          // one piece at a time: the registers go to keeping several polynomial chains in flight instead
+        // one piece at a time (the registers go to keeping several polynomial chains in flight), the chunks in
+        // a rolled loop (the unrolled kernel did not fit the instruction cache)
+#pragma unroll 1
+        for (int ch = 0; ch < n_ch; ++ch) {
           uint32_t r[32];
-          tmem_ld_16x256b_x8(tq, r);
+          tmem_ld_16x256b_x8(tq + ch * 64, r);
           tmem_wait_ld();
-          stats_piece<true, 0>(r, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
-          tmem_ld_16x256b_x8(tq_hi, r);
+          stats_piece<0>(r, zq, lq, cs, qd, hf * kHalf + ch * 64, c_lo, c_hi);
+          tmem_ld_16x256b_x8(tq_hi + ch * 64, r);
           tmem_wait_ld();
-          if (n_ch == 1) release();
-          stats_piece<true, 2>(r, zq, lq, cs, qd, hf * kHalf, c_lo, c_hi);
-          if (n_ch > 1) {
-            tmem_ld_16x256b_x8(tq + 64, r);
-            tmem_wait_ld();
-            stats_piece<false, 0>(r, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
-            tmem_ld_16x256b_x8(tq_hi + 64, r);
-            tmem_wait_ld();
-            release();
-            stats_piece<false, 2>(r, zq, lq, cs, qd, hf * kHalf + 64, c_lo, c_hi);
-          }
-        } else {
-          release();
+          if (ch == n_ch - 1) release();
+          stats_piece<2>(r, zq, lq, cs, qd, hf * kHalf + ch * 64, c_lo, c_hi);
         }
+        if (n_ch == 0) release();
         // ---- reduce-scatter over the 4 lanes of a quad (6 shuffles): lane qd ends up with row k = qd ----
         int z_row;
         float l_row;
@@ -546,7 +545,7 @@ score_tc2_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constan
       const int n_ch = (half_cols(it.n_cols, hf) + 63) >> 6;            // chunks of this half the MMA writes: 0 .. 2
       float* out = c.partial + ((long long)it.unit * c.parts + it.part) * c.n_pad;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
+        const int b = tile_iter & (kSlots - 1), par = (tile_iter / kSlots) & 1;
         mbar_wait(zready + 8 * (b * 4 + q), par);
         float o[4];
 #pragma unroll

@@ -75,6 +75,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       :: "r"(bar), "r"(parity) : "memory");
 }
 #endif
+// one non-blocking probe of a barrier phase (warp-uniform: true if any lane saw the phase complete)
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return __any_sync(0xffffffffu, ok != 0);
+}
 // producer-side wait: polls with a pause, so the spinning warp does not take issue slots from the math warps
 __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
   for (;;) {
