@@ -333,3 +333,66 @@ def test_two_phase_score_kernel_variant(gpu, chk, case):
     stats, _, _ = _parity(gpu, chk, wl, flags_extra=kara.KARA_SCORE_TWO_PHASE)
     assert stats["score_path"] == 3 and stats["s3_hard_mismatch"] == 0
     assert stats["s1_worst_err_over_tol"] < 0.25          # degree-3 exp2: 7.5e-5 of a 1e-3 tolerance
+
+
+@pytest.mark.parametrize("name,L,ratio", [("cfg3", 2, 0.2), ("cfg4", 1, 0.1), ("cfg4", 1, 0.3), ("cfg5", 1, 0.2)])
+def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
+    """BASELINE.json configs[2..4] at their batch sizes, in the launch configuration bench.py times (generated on
+    the device, L resident layers): cfg3 = 64 sequences, histories in [2K, 16K] (not block aligned), block tables
+    permuted over a shared pool — 1,024 units / 20,480 query tiles in one call; cfg4 = 256 sequences, W = 1024
+    (clusters of 4), pool 95 % full, retention 10 % and 30 %; cfg5 = 16 sequences, W = 2048 (clusters of 8),
+    GQA 8, Student-t keys, histories up to 128K.  Properties on every sampled unit, the three-stage check on units
+    computed one by one by the oracle, untouched blocks byte-identical."""
+    kara, gu = gpu
+    from oracle import kara_oracle as ko
+    from oracle import check
+    sh = kin.scaled({"cfg3": kin.CFG3, "cfg4": kin.CFG4, "cfg5": kin.CFG5}[name], ratio=ratio)
+    dev = torch.device("cuda:0")
+    wl = kin.generate(sh, seed=3, device=dev, n_layers_resident=L, history_fill="pattern")
+    S, Hkv, G, n, bs = sh.n_seqs, sh.n_kv_heads, sh.n_q_heads // sh.n_kv_heads, sh.W - sh.U, sh.block_size
+    k0, v0 = wl.k_pool.clone(), wl.v_pool.clone()
+    bt0, sl0, fc0 = wl.block_table.clone(), wl.seq_lens.clone(), int(wl.free_count[0])
+    cache = kara.KaraCache(bs, L, Hkv, sh.head_dim)
+    cache.attach_pool(wl.k_pool, wl.v_pool, wl.free_list, wl.free_count)
+    cache.compress_window(0, L, wl.block_table, wl.seq_lens, wl.win_start, wl.window_q, sh.W, sh.U, sh.ratio,
+                          sh.alpha, sh.gamma, kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    assert cache.status() == 0 and cache.last_score_path() == 2
+    keep = ko.budget(n, sh.ratio)
+    h = wl.win_start.cpu().numpy().astype(np.int64)
+    old_len = sl0.cpu().numpy().astype(np.int64)
+    t = old_len - h - sh.W
+    new_len = h + keep + sh.U + t
+    np.testing.assert_array_equal(wl.seq_lens.cpu().numpy(), new_len)
+    freed = (-(-old_len // bs)) - (-(-new_len // bs))
+    assert int(wl.free_count[0]) - fc0 == int(freed.sum())
+    # blocks no window touches are byte-identical (history never recompressed, PAPER.md:L48)
+    touched = torch.zeros(wl.num_blocks, dtype=torch.bool, device=dev)
+    for s in range(S):
+        touched[bt0[s, int(h[s]) // bs: int(-(-old_len[s] // bs))].long()] = True
+    assert torch.equal(wl.k_pool[:, ~touched], k0[:, ~touched]) and torch.equal(wl.v_pool[:, ~touched], v0[:, ~touched])
+    # every unit: sum_j A_j = G W (sampled over a stride to keep the read-back short), F sorted / unique / in range
+    for u in range(0, L * S * Hkv, 7 if name == "cfg3" else 13):
+        l, s, hk = u // (S * Hkv), (u // Hkv) % S, u % Hkv
+        A = cache.gather_debug(kara.KARA_DBG_SCORES, l, s, hk)
+        F = cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, s, hk)
+        assert abs(float(A.astype(np.float64).sum()) - G * sh.W) <= 1e-4 * G * sh.W
+        assert F.shape[0] == keep and np.all(np.diff(F) > 0) and F[0] >= 0 and F[-1] < n
+    # sampled units against the oracle
+    rng = np.random.default_rng(11)
+    for _ in range(6 if name != "cfg5" else 2):          # (a cfg5 unit is 8.3 GFLOP for the oracle)
+        l, s, hk = int(rng.integers(L)), int(rng.integers(S)), int(rng.integers(Hkv))
+        hs, ols, ts = int(h[s]), int(old_len[s]), int(t[s])
+        q_bits = check.bits(wl.window_q[l, s, :, hk * G:(hk + 1) * G, :])
+        k_old = check.bits(kin.logical_rows(k0, l, bt0[s], ols, hk))
+        v_old = check.bits(kin.logical_rows(v0, l, bt0[s], ols, hk))
+        A64, A32 = ko.scores(q_bits, k_old[hs:hs + n])
+        A = cache.gather_debug(kara.KARA_DBG_SCORES, l, s, hk)
+        assert np.all(np.abs(A.astype(np.float64) - A64) <= check.score_tolerance(A64, G, sh.W, n)), f"S1 {(l, s, hk)}"
+        F = cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, s, hk)
+        np.testing.assert_array_equal(F, ko.select(A, keep, sh.alpha, sh.gamma)["F"])          # S2
+        for what, old in ((kara.KARA_DBG_K_LOGICAL, k_old), (kara.KARA_DBG_V_LOGICAL, v_old)):
+            got = cache.gather_debug(what, l, s, hk, wl.block_table, wl.seq_lens)
+            np.testing.assert_array_equal(got, ko.compact_rows(old, hs, sh.W, sh.U, ts, F))
+        own = ko.select(A32, keep, sh.alpha, sh.gamma)["F"]                                   # S3
+        assert np.array_equal(F, own) or check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 {(l, s, hk)}"
