@@ -82,3 +82,17 @@ def test_binding_fails_loudly_without_the_library(kara, monkeypatch, tmp_path):
     monkeypatch.setattr(kara, "_SO", tmp_path / "missing.so")
     with pytest.raises(kara.KaraError):
         kara.lib()
+
+
+def test_header_constants_match_the_binding(kara):
+    """Every #define of include/kara.h (flags, debug selectors, status bits, error codes) has the same value in the
+    Python binding: the binding marshals arguments, it must not reinterpret them."""
+    text = (ROOT / "include" / "kara.h").read_text()
+    defs = dict(re.findall(r"^#define\s+(KARA_[A-Z0-9_]+)\s+\(?(-?\d+)u?\)?", text, flags=re.M))
+    assert {"KARA_COMMIT", "KARA_KEEP_DEBUG", "KARA_SCORE_QBUF_ONLY", "KARA_SCORE_SIMT", "KARA_SCORE_TWO_PHASE"} <= set(defs)
+    checked = 0
+    for name, val in defs.items():
+        if hasattr(kara, name):
+            assert getattr(kara, name) == int(val), name
+            checked += 1
+    assert checked >= 10
