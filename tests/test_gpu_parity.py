@@ -319,7 +319,7 @@ def test_odd_shapes_against_the_oracle(gpu, chk, W, U, d, G, bs, hist):
     assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
 
 
-@pytest.mark.parametrize("case", ["cfg1", "cfg2x2", "ragged_batch", "w1024"])
+@pytest.mark.parametrize("case", ["cfg1", "cfg2x2", "ragged_batch", "w1024", "w2048_student_t"])
 def test_two_phase_score_kernel_variant(gpu, chk, case):
     """KARA_SCORE_TWO_PHASE (csrc/score_tc2.cu: S computed twice, FMA-pipe exponentials for the row statistics,
     no TMEM write-back) against the oracle: same three-stage parity, same tolerance."""
@@ -329,7 +329,9 @@ def test_two_phase_score_kernel_variant(gpu, chk, case):
           "ragged_batch": lambda: kin.generate(kin.scaled(kin.CFG3, n_seqs=5, n_layers=2, hist_lo=100, hist_hi=900,
                                                           tail_lo=0, tail_hi=15), seed=3),
           "w1024": lambda: kin.generate(kin.scaled(kin.CFG4, n_seqs=2, n_layers=1, hist_lo=50, hist_hi=400,
-                                                   pool_slack=1.1), seed=4)}[case]()
+                                                   pool_slack=1.1), seed=4),
+          "w2048_student_t": lambda: kin.generate(kin.scaled(kin.CFG5, n_seqs=2, n_layers=1, hist_lo=70, hist_hi=500,
+                                                             pool_slack=1.1), seed=5)}[case]()
     stats, _, _ = _parity(gpu, chk, wl, flags_extra=kara.KARA_SCORE_TWO_PHASE)
     assert stats["score_path"] == 3 and stats["s3_hard_mismatch"] == 0
     assert stats["s1_worst_err_over_tol"] < 0.25          # degree-3 exp2: 7.5e-5 of a 1e-3 tolerance
