@@ -208,8 +208,7 @@ def run_gpu(args):
     cache = kara.KaraCache(shape.block_size, L, shape.n_kv_heads, shape.head_dim)
     cache.attach_pool(wl.k_pool, wl.v_pool, wl.free_list, wl.free_count)
     cache.enable_score_timing(not args.no_score_timing)
-    flags = kara.KARA_COMMIT | (kara.KARA_SCORE_SIMT if args.simt else 0) | \
-        (kara.KARA_SCORE_TWO_PHASE if args.two_phase else 0)
+    flags = kara.KARA_COMMIT | (kara.KARA_SCORE_SIMT if args.simt else 0)
     ws = torch.empty(cache.workspace_bytes(L, shape.n_seqs, shape.n_q_heads, shape.W, shape.U, shape.ratio,
                                            shape.alpha), dtype=torch.uint8, device=dev)
     # pristine copies: only the window blocks change, but a full copy is simple and untimed
@@ -298,7 +297,7 @@ def run_gpu(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": _config(args.workload, shape, L, {"score_kernel": {1: "simt", 2: "tcgen05+tma", 3: "tcgen05+tma two-phase"}.get(score_path),
+        "config": _config(args.workload, shape, L, {"score_kernel": {1: "simt", 2: "tcgen05+tma"}.get(score_path),
                                                      "freed_blocks_per_step": freed}),
         "kv_gbs": world * alg["kv_in_bytes"] / (ms_per_step * 1e-3) / 1e9,
         "algorithmic_gbs": world * alg["bytes"] / (ms_per_step * 1e-3) / 1e9,
@@ -340,7 +339,6 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--layers", type=int, default=0, help="resident layers (default: all that fit)")
     ap.add_argument("--simt", action="store_true", help="force the CUDA-core score kernel")
-    ap.add_argument("--two-phase", action="store_true", help="the two-phase tcgen05 score kernel variant (score_tc2.cu)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-score-timing", action="store_true",
                     help="no CUDA events inside the library around the score launch (roofline.kernel_ms = 0)")

@@ -31,7 +31,11 @@
  * Every call returns 0 (KARA_OK) or a negative KARA_E* code and never throws or aborts;
  * kara_last_error() gives a thread-local message for the last failure.  Data-dependent faults
  * found on the device (a block id outside the pool, a sequence shorter than its window) set bits
- * in a device status word, the offending unit is skipped, and kara_status() reports the bits.
+ * in a device status word and the offending SEQUENCE is skipped as a whole: every block-table entry
+ * its window touches is validated before anything is written, so its K/V rows, its block-table row,
+ * its seq_len and the free list stay byte-identical (its debug scores / indices are undefined).  The
+ * check depends on the tables only, so every layer-range call and the committing call skip the same
+ * sequences.  The status word accumulates over the calls of one handle until kara_status() reads it.
  *
  * Physical layout fixed by kara_init_cache (separate K and V pools, each):
  *     bf16 pool[n_layers][num_blocks][n_kv_heads][block_size][head_dim]
@@ -63,8 +67,6 @@ extern "C" {
 #define KARA_KEEP_DEBUG 2u       /* keep scores / I / F of every unit in the workspace for kara_gather_debug */
 #define KARA_SCORE_QBUF_ONLY 4u  /* ablation "w/o Bi-Attention": queries = buffer U only */
 #define KARA_SCORE_SIMT 8u       /* force the CUDA-core score kernel (debug cross-check of the tcgen05 path) */
-#define KARA_SCORE_TWO_PHASE 16u /* tcgen05 score kernel, two-phase variant (S computed twice, no TMEM write-back;
-                                    same results within the score tolerance; csrc/score_tc2.cu) */
 
 /* `what` of kara_gather_debug */
 #define KARA_DBG_K_LOGICAL 0  /* bf16 [seq_len][d] rows of (layer, seq, kv_head) read through the block table */
@@ -79,6 +81,7 @@ extern "C" {
 #define KARA_ST_BAD_BLOCK 1   /* a block-table entry touched by the window is outside [0, num_blocks) */
 #define KARA_ST_SHORT_SEQ 2   /* win_start < 0 or win_start + W > seq_len */
 #define KARA_ST_TABLE_OVERFLOW 4 /* ceil(seq_len / block_size) > max_blocks */
+#define KARA_ST_FREE_OVERFLOW 8  /* a5 would push past free_list[num_blocks) (stale or duplicated free_count) */
 
 typedef struct kara_cache kara_cache;
 
@@ -147,14 +150,15 @@ int kara_gather_debug(kara_cache* c, int what, int layer, int seq, int kv_head,
                       int max_blocks, void* out /*host*/, int64_t out_capacity_bytes,
                       int64_t* out_count /*host*/);
 
-/* Synchronous: reads and clears the device status word of the last call (0 = no fault). */
+/* Synchronous: reads and clears the device status word (0 = no fault).  The word is sticky: it holds the
+ * OR of the faults of every kara_compress_window call on this handle since the last kara_status(), as long
+ * as those calls used the same workspace (the layer-range flow: several calls, KARA_COMMIT on the last). */
 int kara_status(kara_cache* c, int32_t* status_out /*host*/);
 
 /* Number of kernel launches the last kara_compress_window call made (for bench.py's gpu_launches). */
 int kara_last_launch_count(const kara_cache* c);
 
-/* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA,
-   3 = tcgen05/TMA two-phase variant (KARA_SCORE_TWO_PHASE). */
+/* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA. */
 int kara_last_score_path(const kara_cache* c);
 
 /* Device time of the score kernel (a1) alone: when enabled, every kara_compress_window call

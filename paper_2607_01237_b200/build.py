@@ -26,9 +26,17 @@ FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-li
 
 def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
-    hdrs = list(CSRC.glob("*.h")) + [HERE.parent / "include" / "kara.h"]
+    hdrs = list(CSRC.glob("*.h")) + list(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "kara.h"]
     newest_hdr = max(p.stat().st_mtime for p in hdrs)
+    # objects are only reused if they were compiled with the same flags (-D switches change the code)
+    flags_file, flags_now = OBJ / "FLAGS.txt", " ".join(FLAGS)
+    if not flags_file.exists() or flags_file.read_text() != flags_now:
+        force = True
     objs, rebuilt = [], False
+    for stale in OBJ.glob("*.o"):                      # objects of sources that no longer exist
+        if not (CSRC / (stale.stem + ".cu")).exists():
+            stale.unlink()
+            rebuilt = True
     for cu in sorted(CSRC.glob("*.cu")):
         o = OBJ / (cu.stem + ".o")
         objs.append(o)
@@ -41,6 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
                 raise RuntimeError(f"nvcc failed on {cu.name}")
             (OBJ / (cu.stem + ".ptxas.txt")).write_text(r.stderr)
             rebuilt = True
+    flags_file.write_text(flags_now)
     if rebuilt or not SO.exists():
         tmp = SO.with_suffix(f".tmp{os.getpid()}.so")
         cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static",

@@ -24,6 +24,9 @@ struct kara_cache {
   Call last{};
   int last_launches = 0;
   int last_score_path = 0;
+  // sticky device status word: not cleared between the calls of a step (see kara_status)
+  const void* status_ws = nullptr;
+  bool status_pending = false;
   // score-kernel timing
   bool timing = false;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -244,7 +247,11 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   k.free_list = c->free_list;
   k.free_count = c->free_count;
 
-  KARA_CUDA(cudaMemsetAsync(k.status, 0, 8 * sizeof(int32_t), st));
+  // the status word accumulates over the calls of a step (same workspace) until kara_status() reads it
+  if (!(c->status_pending && c->status_ws == workspace))
+    KARA_CUDA(cudaMemsetAsync(k.status, 0, 8 * sizeof(int32_t), st));
+  c->status_ws = workspace;
+  c->status_pending = true;
   int launches = 0;
 
   // ---- a1 score ------------------------------------------------------------------------------
@@ -255,15 +262,9 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   }
   if (use_tc) {
     int nl = 0;
-    if (flags & KARA_SCORE_TWO_PHASE) {
-      rc = score_tc2_launch(&c->tc, k, st, &nl);   // sets k.part_T / part_nc / part_tpu
-      if (rc != KARA_OK) return fail(rc, "score_tc2_launch: %s", score_tc2_error());
-      c->last_score_path = 3;
-    } else {
-      rc = score_tc_launch(&c->tc, k, st, &nl);    // sets k.part_T / part_nc / part_tpu
-      if (rc != KARA_OK) return fail(rc, "score_tc_launch: %s", score_tc_error());
-      c->last_score_path = 2;
-    }
+    rc = score_tc_launch(&c->tc, k, st, &nl);    // sets k.part_T / part_nc / part_tpu
+    if (rc != KARA_OK) return fail(rc, "score_tc_launch: %s", score_tc_error());
+    c->last_score_path = 2;
     launches += nl;
   } else {
     const int rows = (W - k.q_row_begin) * k.G;
@@ -425,6 +426,7 @@ int kara_status(kara_cache* c, int32_t* status_out) {
   KARA_CUDA(cudaDeviceSynchronize());
   KARA_CUDA(cudaMemcpy(status_out, c->last.status, sizeof(int32_t), cudaMemcpyDeviceToHost));
   KARA_CUDA(cudaMemset(c->last.status, 0, sizeof(int32_t)));
+  c->status_pending = false;
   return KARA_OK;
 }
 

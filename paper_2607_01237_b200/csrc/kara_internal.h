@@ -99,6 +99,23 @@ __device__ inline bool window_of(const Call& c, int s, int& h, int& t, int& len)
   return true;
 }
 
+// True if every block-table entry the window of sequence s touches — tokens [h, len), i.e. the rows the
+// compaction reads or writes and the trailing entries a5 may free — is a block id inside the pool.
+// Called by ALL threads of a CTA (contains __syncthreads); sets the status bit on failure.  Depends on the
+// tables only, so every kernel of every call of a step takes the same decision for a sequence.
+__device__ inline bool window_blocks_ok(const Call& c, int s, int h, int len) {
+  const int b0 = h >> c.g.bs_log2, b1 = (len + c.g.bs - 1) >> c.g.bs_log2;
+  const int32_t* row = c.block_table + (long long)s * c.max_blocks;
+  int bad = 0;
+  for (int b = b0 + (int)threadIdx.x; b < b1; b += (int)blockDim.x) {
+    const int blk = row[b];
+    bad |= (blk < 0 || blk >= c.g.num_blocks) ? 1 : 0;
+  }
+  bad = __syncthreads_or(bad);
+  if (bad && threadIdx.x == 0) atomicOr(c.status, KARA_ST_BAD_BLOCK);
+  return !bad;
+}
+
 // Element offset of logical token `pos` of sequence s, head hk, in layer `layer` (absolute).
 // Returns -1 (and sets the status bit) if the block id is outside the pool.
 __device__ inline long long row_offset(const Call& c, int layer, int s, int hk, int pos) {

@@ -32,6 +32,13 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
       old_nb = (len + c.g.bs - 1) >> c.g.bs_log2;
       ok = (h >= 0 && t >= 0 && old_nb <= c.max_blocks);
       if (ok) {
+        // the same validation select_compact ran: a sequence with a block id outside the pool in its window
+        // was not compacted and is not committed (its table row, seq_len and the free list stay as they are)
+        const int32_t* row = c.block_table + (long long)s * c.max_blocks;
+        for (int b = h >> c.g.bs_log2; b < old_nb; ++b) ok &= (row[b] >= 0 && row[b] < c.g.num_blocks);
+        if (!ok) atomicOr(c.status, KARA_ST_BAD_BLOCK);
+      }
+      if (ok) {
         new_len = h + c.keep + c.U + t;
         new_nb = (new_len + c.g.bs - 1) >> c.g.bs_log2;
         freed = old_nb - new_nb;
@@ -52,6 +59,14 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
       tot += warp_tot[w];
     }
     base += inc - freed;
+    // a stale or duplicated free_count must not push past the list: the whole batch of 256 sequences is refused
+    // (uniform decision, so the running count stays consistent) and the status word says why
+    const bool overflow = (long long)s_running + tot > c.g.num_blocks || s_running < 0;
+    if (overflow) {
+      if (tid == 0) atomicOr(c.status, KARA_ST_FREE_OVERFLOW);
+      ok = false;
+      tot = 0;
+    }
     if (ok) {
       int32_t* row = c.block_table + (long long)s * c.max_blocks;
       for (int b = new_nb; b < old_nb; ++b) {

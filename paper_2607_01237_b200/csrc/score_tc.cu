@@ -31,7 +31,7 @@
 //       TMEM load shape the column sum over ALL tiles of a segment is a plain packed FFMA2;
 //       lanes are combined once per segment.
 // TMEM holds two 128 x 256 fp32 S buffers (all 512 columns).  The K panel is double-buffered so a
-// segment change costs no bubble.  score_tc2.cu is the two-phase variant of this kernel.
+// segment change costs no bubble.
 //
 // Warp roles (768 threads): warps 0-15 B (q = warp & 3, cq = warp >> 2), 16-19 C (q = warp & 3),
 // 20 TMA producer, 21 MMA issuer, 22-23 idle (they complete the warpgroup whose registers
@@ -53,7 +53,7 @@ constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works 
 // registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
 // 4 x 72 (B) + 152 (C) + 40 (producer, MMA, idle) = 6 x 80
 constexpr int kRegsB = 72, kRegsC = 152, kRegsOther = 40;
-char g_tc_err[256] = "";
+thread_local char g_tc_err[256] = "";
 
 // ------------------------------------------------------------------------------------------------
 // shared-memory carve-up (dynamic smem, manually aligned to 1024 B for the 128B swizzle)
@@ -232,7 +232,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform for the compiler
   const int rank = CL > 1 ? (int)cluster_ctarank() : 0;
   const int cluster_id = blockIdx.x / CL, n_clusters = gridDim.x / CL;
   const long long g_begin = (long long)cluster_id * T / n_clusters;
@@ -637,12 +637,9 @@ template <int D, int CL>
 int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
   using SM = Smem<D, CL>;
   auto kern = score_tc_kernel<D, CL>;
-  static bool attr_done = false;
-  if (!attr_done) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kAlloc) != cudaSuccess)
-      return tc_fail(KARA_ECUDA, "cudaFuncSetAttribute(max dynamic smem) failed");
-    attr_done = true;
-  }
+  // per launch: the attribute belongs to the current device / context, not to the process
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kAlloc) != cudaSuccess)
+    return tc_fail(KARA_ECUDA, "cudaFuncSetAttribute(max dynamic smem) failed");
   const int tok_tiles = (c.W - c.q_row_begin + kTileM - 1) / kTileM;
   const int tpu = tok_tiles * c.G;
   const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;

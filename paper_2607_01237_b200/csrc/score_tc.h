@@ -20,8 +20,5 @@ bool score_tc_supported(const ScoreTcState& s, const Call& c);
 // Launches the kernel(s); sets c.parts to the number of partial column-sum strips it writes.
 int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches);
 const char* score_tc_error();
-// The two-phase variant (score_tc2.cu, KARA_SCORE_TWO_PHASE): same state, same shapes, same outputs.
-int score_tc2_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches);
-const char* score_tc2_error();
 
 }  // namespace kara

@@ -177,6 +177,9 @@ __global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call 
 
   int h, t, len;
   if (!window_of(c, s, h, t, len)) return;   // uniform per CTA
+  // every table entry of the window is validated BEFORE anything is written: a sequence with a block id
+  // outside the pool is skipped as a whole (no compaction here, no metadata update in a5)
+  if (!window_blocks_ok(c, s, h, len)) return;
 
   // ---- scores: sum the score kernel's partial column sums in part order -------------------
   const float* part = c.partial + (long long)unit * c.parts * n_pad;

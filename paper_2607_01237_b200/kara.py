@@ -18,10 +18,10 @@ _SO = _HERE / "libkara.so"
 _LIB = None
 
 KARA_OK, KARA_EINVAL, KARA_EBUDGET, KARA_EUNSUPPORTED, KARA_ECUDA, KARA_ENOMEM = 0, -1, -2, -3, -4, -5
-KARA_COMMIT, KARA_KEEP_DEBUG, KARA_SCORE_QBUF_ONLY, KARA_SCORE_SIMT, KARA_SCORE_TWO_PHASE = 1, 2, 4, 8, 16
+KARA_COMMIT, KARA_KEEP_DEBUG, KARA_SCORE_QBUF_ONLY, KARA_SCORE_SIMT = 1, 2, 4, 8
 (KARA_DBG_K_LOGICAL, KARA_DBG_V_LOGICAL, KARA_DBG_SCORES, KARA_DBG_IDX_TOPK, KARA_DBG_IDX_FINAL,
  KARA_DBG_BLOCK_TABLE_ROW, KARA_DBG_FREE_LIST) = range(7)
-KARA_ST_BAD_BLOCK, KARA_ST_SHORT_SEQ, KARA_ST_TABLE_OVERFLOW = 1, 2, 4
+KARA_ST_BAD_BLOCK, KARA_ST_SHORT_SEQ, KARA_ST_TABLE_OVERFLOW, KARA_ST_FREE_OVERFLOW = 1, 2, 4, 8
 
 # every symbol include/kara.h declares: (restype, argtypes)
 _vp, _i, _i64, _sz, _d, _u = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_double, C.c_uint

@@ -89,7 +89,7 @@ def test_header_constants_match_the_binding(kara):
     Python binding: the binding marshals arguments, it must not reinterpret them."""
     text = (ROOT / "include" / "kara.h").read_text()
     defs = dict(re.findall(r"^#define\s+(KARA_[A-Z0-9_]+)\s+\(?(-?\d+)u?\)?", text, flags=re.M))
-    assert {"KARA_COMMIT", "KARA_KEEP_DEBUG", "KARA_SCORE_QBUF_ONLY", "KARA_SCORE_SIMT", "KARA_SCORE_TWO_PHASE"} <= set(defs)
+    assert {"KARA_COMMIT", "KARA_KEEP_DEBUG", "KARA_SCORE_QBUF_ONLY", "KARA_SCORE_SIMT"} <= set(defs)
     checked = 0
     for name, val in defs.items():
         if hasattr(kara, name):

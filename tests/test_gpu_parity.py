@@ -186,6 +186,70 @@ def test_device_status_word_flags_bad_inputs(gpu):
     assert out["status"] & kara.KARA_ST_SHORT_SEQ
 
 
+def test_bad_block_sequence_is_skipped_as_a_whole(gpu, chk):
+    """include/kara.h: a sequence whose window touches a block id outside the pool is skipped before anything is
+    written: its K/V blocks, its block-table row, its seq_len stay byte-identical and nothing of it reaches the
+    free list; the other sequences of the batch come out exactly as the oracle computes them without it."""
+    kara, gu = gpu
+    shape = kin.scaled(kin.CFG3, n_seqs=3, n_layers=2, hist_lo=100, hist_hi=700, tail_lo=0, tail_hi=9)
+    wl = kin.generate(shape, seed=31)
+    sh, bs = wl.shape, wl.shape.block_size
+    bad_s = 1
+    h, ln = int(wl.win_start[bad_s]), int(wl.seq_lens[bad_s])
+    D = gu.to_cuda(wl)
+    bad_entry = h // bs + 3
+    D["bt"][bad_s, bad_entry] = wl.num_blocks + 5
+    bt_in = D["bt"].cpu().numpy().copy()
+    for tc_path in (True, False):
+        Dr = {k: v.clone() for k, v in D.items()}
+        flags = kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG | (0 if tc_path else kara.KARA_SCORE_SIMT)
+        out, cache, _ = gu.gpu_compress(wl, dev_tensors=Dr, flags=flags)
+        assert out["status"] & kara.KARA_ST_BAD_BLOCK
+        # the offending sequence: nothing of it changed
+        np.testing.assert_array_equal(out["bt"][bad_s], bt_in[bad_s])
+        assert out["sl"][bad_s] == ln
+        H0 = chk.host_image(wl)
+        own_blocks = [int(b) for b in wl.block_table[bad_s, :(ln + bs - 1) // bs] if 0 <= int(b) < wl.num_blocks]
+        np.testing.assert_array_equal(out["k"][:, own_blocks], H0["k"][:, own_blocks])
+        np.testing.assert_array_equal(out["v"][:, own_blocks], H0["v"][:, own_blocks])
+        # the rest of the batch: the oracle on the same pools with that sequence left out
+        keep_rows = [s for s in range(sh.n_seqs) if s != bad_s]
+        Hs = {k_: v_.copy() for k_, v_ in H0.items()}
+        Hs["bt"], Hs["sl"], Hs["ws"] = H0["bt"][keep_rows].copy(), H0["sl"][keep_rows].copy(), H0["ws"][keep_rows].copy()
+        Hs["q"] = np.ascontiguousarray(H0["q"][:, keep_rows])
+        sc = np.ascontiguousarray(out["scores"][:, keep_rows], np.float32)
+        chk.run_oracle(Hs, sh.n_q_heads, sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma, 0, 2, True, scores_in=sc)
+        np.testing.assert_array_equal(out["bt"][keep_rows], Hs["bt"])
+        np.testing.assert_array_equal(out["sl"][keep_rows], Hs["sl"])
+        np.testing.assert_array_equal(out["fc"], Hs["fc"])
+        nfree = int(Hs["fc"][0])
+        np.testing.assert_array_equal(out["fl"][:nfree], Hs["fl"][:nfree])
+        assert np.all((out["fl"][:nfree] >= 0) & (out["fl"][:nfree] < wl.num_blocks))
+        np.testing.assert_array_equal(out["k"], Hs["k"])
+        np.testing.assert_array_equal(out["v"], Hs["v"])
+
+
+def test_status_word_is_sticky_across_layer_range_calls(gpu):
+    """kara_status: a fault of an earlier layer-range call is still reported after the committing call."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_layers=2), seed=3)
+    sh = wl.shape
+    D = gu.to_cuda(wl)
+    cache = kara.KaraCache(sh.block_size, 2, sh.n_kv_heads, sh.head_dim)
+    cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+    ws = torch.empty(cache.workspace_bytes(1, sh.n_seqs, sh.n_q_heads, sh.W, sh.U, sh.ratio, sh.alpha),
+                     dtype=torch.uint8, device="cuda")
+    good = D["bt"].clone()
+    D["bt"][0, 17] = wl.num_blocks + 5
+    cache.compress_window(0, 1, D["bt"], D["sl"], D["ws"], D["q"][0:1].contiguous(), sh.W, sh.U, sh.ratio, sh.alpha,
+                          sh.gamma, 0, workspace=ws)
+    D["bt"].copy_(good)                                     # the table is repaired before the last layer
+    cache.compress_window(1, 2, D["bt"], D["sl"], D["ws"], D["q"][1:2].contiguous(), sh.W, sh.U, sh.ratio, sh.alpha,
+                          sh.gamma, kara.KARA_COMMIT, workspace=ws)
+    assert cache.status() & kara.KARA_ST_BAD_BLOCK          # not erased by the second call
+    assert cache.status() == 0                              # read-and-clear
+
+
 def test_argument_errors_are_reported_not_thrown(gpu):
     kara, gu = gpu
     wl = kin.generate(kin.CFG1, seed=1)
@@ -317,24 +381,6 @@ def test_odd_shapes_against_the_oracle(gpu, chk, W, U, d, G, bs, hist):
                        W=W, U=U, alpha=8, gamma=6, hist_lo=hist, hist_hi=hist + 3 * bs, planted_positions=4)
     stats, _, _ = _parity(gpu, chk, kin.generate(shape, seed=W + U))
     assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
-
-
-@pytest.mark.parametrize("case", ["cfg1", "cfg2x2", "ragged_batch", "w1024", "w2048_student_t"])
-def test_two_phase_score_kernel_variant(gpu, chk, case):
-    """KARA_SCORE_TWO_PHASE (csrc/score_tc2.cu: S computed twice, FMA-pipe exponentials for the row statistics,
-    no TMEM write-back) against the oracle: same three-stage parity, same tolerance."""
-    kara, _ = gpu
-    wl = {"cfg1": lambda: kin.generate(kin.CFG1, seed=5),
-          "cfg2x2": lambda: kin.generate(kin.scaled(kin.CFG2, n_layers=2), seed=2),
-          "ragged_batch": lambda: kin.generate(kin.scaled(kin.CFG3, n_seqs=5, n_layers=2, hist_lo=100, hist_hi=900,
-                                                          tail_lo=0, tail_hi=15), seed=3),
-          "w1024": lambda: kin.generate(kin.scaled(kin.CFG4, n_seqs=2, n_layers=1, hist_lo=50, hist_hi=400,
-                                                   pool_slack=1.1), seed=4),
-          "w2048_student_t": lambda: kin.generate(kin.scaled(kin.CFG5, n_seqs=2, n_layers=1, hist_lo=70, hist_hi=500,
-                                                             pool_slack=1.1), seed=5)}[case]()
-    stats, _, _ = _parity(gpu, chk, wl, flags_extra=kara.KARA_SCORE_TWO_PHASE)
-    assert stats["score_path"] == 3 and stats["s3_hard_mismatch"] == 0
-    assert stats["s1_worst_err_over_tol"] < 0.25          # degree-3 exp2: 7.5e-5 of a 1e-3 tolerance
 
 
 @pytest.mark.parametrize("name,L,ratio", [("cfg3", 2, 0.2), ("cfg4", 1, 0.1), ("cfg4", 1, 0.3), ("cfg5", 1, 0.2)])
