@@ -43,13 +43,13 @@ def layout_of(k_pool_shape) -> ko.Layout:
 
 
 def run_oracle(H: dict, n_q_heads, W, U, ratio, alpha, gamma, layer_begin, layer_end, commit=True,
-               scores_in=None) -> dict:
+               scores_in=None, n_windows=1) -> dict:
     """Runs O1-O11 (or O4-O11 from scores_in) IN PLACE on the numpy image H; returns the dumps."""
     lay = layout_of(H["k"].shape)
     q = None if scores_in is not None else np.ascontiguousarray(H["q"][layer_begin:layer_end])
     return ko.compress_window(lay, H["k"], H["v"], layer_begin, layer_end, H["bt"], H["sl"], H["ws"], q,
                               n_q_heads, W, U, ratio, alpha, gamma, commit, H["fl"], H["fc"],
-                              scores_in=scores_in)
+                              scores_in=scores_in, n_windows=n_windows)
 
 
 def score_tolerance(A_ref: np.ndarray, G: int, W: int, n: int) -> np.ndarray:
@@ -90,7 +90,7 @@ def is_ambiguous(A32: np.ndarray, keep: int, alpha: int, gamma: int, rel: float 
 
 
 def compare(H0: dict, gpu: dict, n_q_heads, W, U, ratio, alpha, gamma, layer_begin, layer_end,
-            commit=True, check_s1=True) -> dict:
+            commit=True, check_s1=True, n_windows=1) -> dict:
     """H0: pristine numpy image.  gpu: numpy read-backs of the CUDA path after its call:
     k, v (pool bits), bt, sl, fl, fc, scores [L,S,Hkv,n], idx_topk [..,k], idx_final [..,keep].
     Raises AssertionError on any parity failure; returns statistics."""
@@ -100,8 +100,13 @@ def compare(H0: dict, gpu: dict, n_q_heads, W, U, ratio, alpha, gamma, layer_beg
     stats = {}
     # ---- oracle on its own scores (S1, S3) ----
     Ho = {k_: v_.copy() for k_, v_ in H0.items()}
-    own = run_oracle(Ho, n_q_heads, W, U, ratio, alpha, gamma, layer_begin, layer_end, commit)
+    own = run_oracle(Ho, n_q_heads, W, U, ratio, alpha, gamma, layer_begin, layer_end, commit, n_windows=n_windows)
     keep = own["keep"]
+    if n_windows > 1:      # the GPU read-backs are [L, S, NW, Hkv, .] too; fold (S, NW) into one axis for the loops below
+        own = {k_: (v_.reshape((v_.shape[0], -1) + v_.shape[3:]) if isinstance(v_, np.ndarray) else v_) for k_, v_ in own.items()}
+        gpu = dict(gpu)
+        for k_ in ("scores", "idx_topk", "idx_final"):
+            gpu[k_] = gpu[k_].reshape((gpu[k_].shape[0], -1) + gpu[k_].shape[3:])
     if check_s1:
         err = np.abs(gpu["scores"].astype(np.float64) - own["scores"].astype(np.float64))
         tol = score_tolerance(own["scores"].astype(np.float64), G, W, n)
@@ -112,7 +117,9 @@ def compare(H0: dict, gpu: dict, n_q_heads, W, U, ratio, alpha, gamma, layer_beg
     # ---- S2: oracle from the GPU's scores must reproduce everything bit for bit ----
     Hs = {k_: v_.copy() for k_, v_ in H0.items()}
     inj = run_oracle(Hs, n_q_heads, W, U, ratio, alpha, gamma, layer_begin, layer_end, commit,
-                     scores_in=np.ascontiguousarray(gpu["scores"], np.float32))
+                     scores_in=np.ascontiguousarray(gpu["scores"], np.float32), n_windows=n_windows)
+    if n_windows > 1:
+        inj = {k_: (v_.reshape((v_.shape[0], -1) + v_.shape[3:]) if isinstance(v_, np.ndarray) else v_) for k_, v_ in inj.items()}
     np.testing.assert_array_equal(gpu["idx_topk"], inj["idx_topk"], err_msg="S2: I differs")
     np.testing.assert_array_equal(gpu["idx_final"], inj["idx_final"], err_msg="S2: F differs")
     np.testing.assert_array_equal(gpu["k"], Hs["k"], err_msg="S2: K pool bytes differ")

@@ -309,3 +309,121 @@ done:
   free(kwin); free(A32); free(I); free(F); free(tmp);
   return rc;
 }
+
+/* ---------------------------------------------------------------------------------------- */
+/* App. C.2 prefill: "partition the prompt into multiple windows of length |W|
+ * and perform window-wise compression on the KV pairs corresponding to positions inside each
+ * window in parallel".  Reading G17: the NW windows of a sequence are the disjoint
+ * ranges [h + w W, h + (w+1) W), each scored with its own W queries against its own n keys and
+ * selected on its own (O1-O9 unchanged); the retained rows and the buffer of window w are laid
+ * down behind those of window w-1, the tail behind the last window:
+ *   new[h + w (keep+U) + c]        = old[h + w W + F_w[c]]       c < keep
+ *   new[h + w (keep+U) + keep + c] = old[h + w W + n + c]        c < U
+ *   new[h + NW (keep+U) + c]       = old[h + NW W + c]           c < t
+ * Unit order of every dump: ((layer, sequence), window, KV head). */
+int kara_oracle_compress_windows(const kara_oracle_layout* lay, uint16_t* k_pool, uint16_t* v_pool,
+                                 int layer_begin, int layer_end, int n_seqs,
+                                 int32_t* block_table, int max_blocks, int32_t* seq_lens,
+                                 const int32_t* win_start, int n_windows,
+                                 const uint16_t* window_q, int n_q_heads,
+                                 int W, int U, double ratio, int alpha, int gamma, int commit,
+                                 int32_t* free_list, int32_t* free_count,
+                                 const float* scores_in, float* scores_out,
+                                 int32_t* idx_topk_out, int32_t* idx_final_out) {
+  if (!lay || !k_pool || !v_pool || !block_table || !seq_lens) return KARA_ORACLE_EINVAL;
+  if (!window_q && !scores_in) return KARA_ORACLE_EINVAL;
+  const int d = lay->head_dim, Hkv = lay->n_kv_heads, bs = lay->block_size;
+  if (layer_begin < 0 || layer_end > lay->n_layers || layer_begin >= layer_end) return KARA_ORACLE_EINVAL;
+  if (n_q_heads % Hkv != 0 || U < 0 || W <= U || n_windows < 1) return KARA_ORACLE_EINVAL;
+  const int G = n_q_heads / Hkv, NW = n_windows;
+  const int n = W - U;
+  const int keep = kara_oracle_budget(n, ratio);
+  if (keep < 0) return KARA_ORACLE_EINVAL;
+  const int k = keep - alpha;
+  if (gamma < 3 || k < 1 || keep > n) return KARA_ORACLE_EBUDGET;
+  const int nL = layer_end - layer_begin;
+  const int per = keep + U;                       /* rows one window leaves behind */
+
+  uint16_t* kwin = (uint16_t*)malloc(sizeof(uint16_t) * (size_t)n * d);
+  float* A32 = (float*)malloc(sizeof(float) * (size_t)n);
+  int32_t* I = (int32_t*)malloc(sizeof(int32_t) * (size_t)k);
+  int32_t* F = (int32_t*)malloc(sizeof(int32_t) * (size_t)keep * NW);
+  uint16_t* tmp = NULL;
+  int rc = KARA_ORACLE_OK;
+  if (!kwin || !A32 || !I || !F) { rc = KARA_ORACLE_EINVAL; goto done; }
+
+  for (int li = 0; li < nL && rc == KARA_ORACLE_OK; ++li) {
+    const int layer = layer_begin + li;
+    for (int s = 0; s < n_seqs && rc == KARA_ORACLE_OK; ++s) {
+      const int len = seq_lens[s];
+      const int h = win_start ? win_start[s] : len - NW * W;
+      const int t = len - h - NW * W;
+      if (h < 0 || t < 0 || ceil_div(len, bs) > max_blocks) { rc = KARA_ORACLE_EINVAL; break; }
+      const int32_t* bt_row = block_table + (long)s * max_blocks;
+      const int moved = NW * per + t;
+      tmp = (uint16_t*)realloc(tmp, sizeof(uint16_t) * (size_t)(moved > 0 ? moved : 1) * d);
+      if (!tmp) { rc = KARA_ORACLE_EINVAL; break; }
+      for (int hk = 0; hk < Hkv && rc == KARA_ORACLE_OK; ++hk) {
+        for (int w = 0; w < NW; ++w) {            /* O1-O9 per window, independently */
+          const long unit = (((long)li * n_seqs + s) * NW + w) * Hkv + hk;
+          const int hw = h + w * W;
+          if (scores_in) {
+            memcpy(A32, scores_in + unit * n, sizeof(float) * (size_t)n);
+          } else {
+            for (int j = 0; j < n; ++j)
+              memcpy(kwin + (size_t)j * d, row_ptr(lay, k_pool, layer, bt_row, hw + j, hk),
+                     sizeof(uint16_t) * (size_t)d);
+            const uint16_t* q = window_q + ((((long)li * n_seqs + s) * NW + w) * W) * n_q_heads * d +
+                                (long)hk * G * d;
+            rc = kara_oracle_scores(q, (long)n_q_heads * d, d, kwin, d, W, G, n, d, NULL, A32);
+            if (rc) break;
+          }
+          if (scores_out) memcpy(scores_out + unit * n, A32, sizeof(float) * (size_t)n);
+          rc = kara_oracle_select(A32, n, keep, alpha, gamma, I, NULL, F + (size_t)w * keep, NULL);
+          if (rc) break;
+          if (idx_topk_out) memcpy(idx_topk_out + unit * k, I, sizeof(int32_t) * (size_t)k);
+          if (idx_final_out)
+            memcpy(idx_final_out + unit * keep, F + (size_t)w * keep, sizeof(int32_t) * (size_t)keep);
+        }
+        if (rc) break;
+        /* O10 over all windows of this (layer, head): gather, then lay down densely */
+        for (int which = 0; which < 2; ++which) {
+          uint16_t* pool = which == 0 ? k_pool : v_pool;
+          for (int w = 0; w < NW; ++w) {
+            for (int c = 0; c < keep; ++c)
+              memcpy(tmp + (size_t)(w * per + c) * d,
+                     row_ptr(lay, pool, layer, bt_row, h + w * W + F[(size_t)w * keep + c], hk),
+                     sizeof(uint16_t) * (size_t)d);
+            for (int c = 0; c < U; ++c)
+              memcpy(tmp + (size_t)(w * per + keep + c) * d,
+                     row_ptr(lay, pool, layer, bt_row, h + w * W + n + c, hk), sizeof(uint16_t) * (size_t)d);
+          }
+          for (int c = 0; c < t; ++c)
+            memcpy(tmp + (size_t)(NW * per + c) * d, row_ptr(lay, pool, layer, bt_row, h + NW * W + c, hk),
+                   sizeof(uint16_t) * (size_t)d);
+          for (int c = 0; c < moved; ++c)
+            memcpy(row_ptr(lay, pool, layer, bt_row, h + c, hk), tmp + (size_t)c * d,
+                   sizeof(uint16_t) * (size_t)d);
+        }
+      }
+    }
+  }
+  if (rc == KARA_ORACLE_OK && commit) {
+    /* O11 with new_len = h + NW (keep+U) + t: trailing table entries freed in table order, batch order */
+    for (int s = 0; s < n_seqs; ++s) {
+      const int len = seq_lens[s];
+      const int h = win_start ? win_start[s] : len - NW * W;
+      const int t = len - h - NW * W;
+      const int new_len = h + NW * per + t;
+      const int old_nb = ceil_div(len, bs), new_nb = ceil_div(new_len, bs);
+      for (int b = new_nb; b < old_nb; ++b) {
+        free_list[(*free_count)++] = block_table[(long)s * max_blocks + b];
+        block_table[(long)s * max_blocks + b] = -1;
+      }
+      seq_lens[s] = new_len;
+    }
+  }
+done:
+  free(kwin); free(A32); free(I); free(F); free(tmp);
+  return rc;
+}

@@ -123,6 +123,22 @@ int kara_oracle_compress_window(const kara_oracle_layout* lay, uint16_t* k_pool,
                                 const float* scores_in, float* scores_out,
                                 int32_t* idx_topk_out, int32_t* idx_final_out);
 
+/* Prefill (App. C.2; reading G17): n_windows disjoint windows of W tokens per
+ * sequence starting at win_start[s] (NULL => seq_len - n_windows*W), each compressed on its own
+ * (O1-O9), retained rows + buffer of window w laid down behind those of window w-1, tail last;
+ * new_len = h + n_windows*(keep+U) + t.  window_q is [layers][n_seqs][n_windows*W][n_q_heads][d];
+ * dumps and scores_in are ordered ((layer, sequence), window, KV head).  n_windows = 1 is
+ * kara_oracle_compress_window. */
+int kara_oracle_compress_windows(const kara_oracle_layout* lay, uint16_t* k_pool, uint16_t* v_pool,
+                                 int layer_begin, int layer_end, int n_seqs,
+                                 int32_t* block_table, int max_blocks, int32_t* seq_lens,
+                                 const int32_t* win_start, int n_windows,
+                                 const uint16_t* window_q, int n_q_heads,
+                                 int W, int U, double ratio, int alpha, int gamma, int commit,
+                                 int32_t* free_list, int32_t* free_count,
+                                 const float* scores_in, float* scores_out,
+                                 int32_t* idx_topk_out, int32_t* idx_final_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -75,6 +75,11 @@ def lib() -> C.CDLL:
             C.POINTER(Layout), u16p, u16p, C.c_int, C.c_int, C.c_int, i32p, C.c_int, i32p, i32p,
             u16p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int,
             i32p, i32p, f32p, f32p, i32p, i32p]
+        L.kara_oracle_compress_windows.restype = C.c_int
+        L.kara_oracle_compress_windows.argtypes = [
+            C.POINTER(Layout), u16p, u16p, C.c_int, C.c_int, C.c_int, i32p, C.c_int, i32p, i32p, C.c_int,
+            u16p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int,
+            i32p, i32p, f32p, f32p, i32p, i32p]
         _LIB = L
     return _LIB
 
@@ -163,8 +168,9 @@ def metadata(block_table, seq_lens, win_start, block_size, W, U, keep, free_list
 
 def compress_window(layout: Layout, k_pool, v_pool, layer_begin, layer_end, block_table, seq_lens,
                     win_start, window_q, n_q_heads, W, U, ratio, alpha, gamma, commit,
-                    free_list, free_count, scores_in=None, want_debug=True):
+                    free_list, free_count, scores_in=None, want_debug=True, n_windows=1):
     """Whole path O1-O11 on host images (all modified in place).  Returns dict of debug dumps.
+    n_windows > 1: prefill, kara_oracle_compress_windows (dumps get a window axis after the sequence axis).
 
     k_pool / v_pool: uint16 numpy (bf16 bits), any shape, addressed through `layout` strides.
     window_q: uint16 [layers, n_seqs, W, n_q_heads, d] or None when scores_in is given.
@@ -186,11 +192,24 @@ def compress_window(layout: Layout, k_pool, v_pool, layer_begin, layer_end, bloc
     units = nL * n_seqs * layout.n_kv_heads
     out = {"keep": keep, "k": k}
     s_out = i_out = f_out = None
+    NW = int(n_windows)
+    lead = (nL, n_seqs) if NW == 1 else (nL, n_seqs, NW)
     if want_debug:
-        s_out = np.zeros((nL, n_seqs, layout.n_kv_heads, n), np.float32)
-        i_out = np.full((nL, n_seqs, layout.n_kv_heads, max(k, 1)), -1, np.int32)
-        f_out = np.full((nL, n_seqs, layout.n_kv_heads, max(keep, 1)), -1, np.int32)
+        s_out = np.zeros(lead + (layout.n_kv_heads, n), np.float32)
+        i_out = np.full(lead + (layout.n_kv_heads, max(k, 1)), -1, np.int32)
+        f_out = np.full(lead + (layout.n_kv_heads, max(keep, 1)), -1, np.int32)
     del units
+    if NW > 1:
+        rc = lib().kara_oracle_compress_windows(
+            C.byref(layout), _p(k_pool, C.c_uint16), _p(v_pool, C.c_uint16), layer_begin, layer_end,
+            n_seqs, _p(block_table, C.c_int32), max_blocks, _p(seq_lens, C.c_int32),
+            _p(win_start, C.c_int32), NW, _p(window_q, C.c_uint16), n_q_heads, W, U, float(ratio),
+            alpha, gamma, int(bool(commit)), _p(free_list, C.c_int32), _p(free_count, C.c_int32),
+            _p(scores_in, C.c_float), _p(s_out, C.c_float), _p(i_out, C.c_int32), _p(f_out, C.c_int32))
+        if rc:
+            raise ValueError(f"kara_oracle_compress_windows rc={rc}")
+        out.update(scores=s_out, idx_topk=i_out, idx_final=f_out)
+        return out
     rc = lib().kara_oracle_compress_window(
         C.byref(layout), _p(k_pool, C.c_uint16), _p(v_pool, C.c_uint16), layer_begin, layer_end,
         n_seqs, _p(block_table, C.c_int32), max_blocks, _p(seq_lens, C.c_int32),

@@ -51,6 +51,7 @@ class KaraShape:
     run_lo: int = 2
     run_hi: int = 16
     pool_slack: float = 1.2      # num_blocks = ceil(slack * live blocks)
+    n_windows: int = 1           # prefill (App. C.2): this many disjoint windows of W tokens per sequence
 
     @property
     def n(self) -> int:
@@ -73,7 +74,11 @@ CFG4 = KaraShape("cfg4_serving256", 256, 40, 40, 8, 128, 16, W=1024, U=32, ratio
 CFG5 = KaraShape("cfg5_longcot", 16, 64, 64, 8, 128, 16, W=2048, U=64, ratio=0.2, alpha=32, gamma=8,
                  hist_lo=65536, hist_hi=131072, k_dist="student_t3", salient_frac=0.05, run_lo=1,
                  run_hi=64)
-CONFIGS = {c.name: c for c in (CFG1, CFG2, CFG3, CFG4, CFG5)}
+# a prompt split into windows of W and compressed in one call: 8 prompts of
+# 16 x 512 tokens, no compressed history in front, same attention shape and hyper-parameters as cfg 2/3.
+PREFILL = KaraShape("prefill_8x16x512", 8, 40, 40, 8, 128, 16, W=512, U=32, ratio=0.2, alpha=32, gamma=8,
+                    hist_lo=0, hist_hi=0, salient_frac=0.05, n_windows=16)
+CONFIGS = {c.name: c for c in (CFG1, CFG2, CFG3, CFG4, CFG5, PREFILL)}
 
 
 def scaled(shape: KaraShape, **kw) -> KaraShape:
@@ -90,7 +95,7 @@ class Workload:
     max_blocks: int
     k_pool: torch.Tensor          # bf16 [L, NB, Hkv, bs, d]
     v_pool: torch.Tensor
-    window_q: torch.Tensor        # bf16 [L, S, W, Hq, d]
+    window_q: torch.Tensor        # bf16 [L, S, n_windows * W, Hq, d]
     block_table: torch.Tensor     # int32 [S, max_blocks], -1 padded
     seq_lens: torch.Tensor        # int32 [S]
     win_start: torch.Tensor       # int32 [S]
@@ -135,6 +140,7 @@ def generate(shape: KaraShape, seed: int, device: str | torch.device = "cpu",
     dev = torch.device(device)
     L = shape.n_layers if n_layers_resident is None else int(n_layers_resident)
     S, W, U, n = shape.n_seqs, shape.W, shape.U, shape.n
+    NW = shape.n_windows
     Hq, Hkv, d, bs, G = shape.n_q_heads, shape.n_kv_heads, shape.head_dim, shape.block_size, shape.G
     cg = torch.Generator(device="cpu").manual_seed(int(seed))
     vg = torch.Generator(device=dev).manual_seed(int(seed) ^ 0x5DEECE66D)
@@ -142,7 +148,7 @@ def generate(shape: KaraShape, seed: int, device: str | torch.device = "cpu",
     # ---- structure: lengths, block tables, free list (CPU, exact integers) -------------------
     h = torch.randint(shape.hist_lo, shape.hist_hi + 1, (S,), generator=cg, dtype=torch.int64)
     t = torch.randint(shape.tail_lo, shape.tail_hi + 1, (S,), generator=cg, dtype=torch.int64)
-    seq_len = h + W + t
+    seq_len = h + NW * W + t
     nblk = (seq_len + bs - 1) // bs
     live = int(nblk.sum())
     num_blocks = max(int(math.ceil(shape.pool_slack * live)), live)
@@ -163,7 +169,7 @@ def generate(shape: KaraShape, seed: int, device: str | torch.device = "cpu",
     # ---- values ------------------------------------------------------------------------------
     k_pool = torch.empty((L, num_blocks, Hkv, bs, d), dtype=torch.bfloat16, device=dev)
     v_pool = torch.empty_like(k_pool)
-    window_q = torch.empty((L, S, W, Hq, d), dtype=torch.bfloat16, device=dev)
+    window_q = torch.empty((L, S, NW * W, Hq, d), dtype=torch.bfloat16, device=dev)
     out_ch = torch.randperm(d, generator=cg)[: shape.n_outlier_channels].to(dev)
     bt_dev = block_table.to(dev).long()
     sal_dev = salient.to(dev)
@@ -194,13 +200,14 @@ def generate(shape: KaraShape, seed: int, device: str | torch.device = "cpu",
         else:
             raise ValueError(history_fill)
         for s in range(S):
-            # window queries: N(0,1) + c * v_hat per (layer, seq, kv head)
+          for w in range(NW):
+            # window queries: N(0,1) + c * v_hat per (layer, seq, window, kv head)
             v_hat = _unit(randn(Hkv, d))
             q = randn(W, Hkv, G, d) + shape.q_shift * v_hat[None, :, None, :]
             q_bf = q.to(torch.bfloat16)
-            window_q[l, s] = q_bf.view(W, Hq, d)
-            # window + tail keys / values
-            wt = W + int(t[s])
+            window_q[l, s, w * W:(w + 1) * W] = q_bf.view(W, Hq, d)
+            # window (+ tail behind the last window) keys / values
+            wt = W + (int(t[s]) if w == NW - 1 else 0)
             kw = draw_k(wt, Hkv, d)
             vw = randn(wt, Hkv, d)
             if bool(salient[s].any()):
@@ -212,7 +219,7 @@ def generate(shape: KaraShape, seed: int, device: str | torch.device = "cpu",
                 orth = _unit(kc - (kc * u_hat).sum(-1, keepdim=True) * u_hat)
                 planted = nrm * (0.8 * u_hat + 0.6 * orth)
                 kw[:n] = torch.where(sal_dev[s][:, None, None], planted, kc)
-            pos = torch.arange(int(h[s]), int(h[s]) + wt, device=dev)
+            pos = torch.arange(int(h[s]) + w * W, int(h[s]) + w * W + wt, device=dev)
             blk = bt_dev[s, pos // bs]
             slot = pos % bs
             k_pool[l, blk, :, slot, :] = kw.to(torch.bfloat16)
