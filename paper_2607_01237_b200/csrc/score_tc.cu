@@ -14,28 +14,26 @@
 //   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM,
 //       issued as two N <= 128 halves, each with its own full / empty barrier, so a half is
 //       refilled as soon as its column sums have been taken.
-//   The softmax is split over SPECIALISED warps (the v2 kernel ran both passes in the same warps
-//   and was bound by the latency of its own dependency chain, 2 warps per sub-partition):
+//   The softmax is split over SPECIALISED warps, none of which waits for more than one thing:
 //   B warps (16: TMEM lane quadrant q x 64-column chunk cq) — pass B, the only MUFU work.  One TMEM
-//       read, one write: a thread holds 2 rows x 16 columns per piece (two pieces per tile); it shifts
-//       by ITS OWN maximum of those 16 logits, rounded to an integer z (log2 domain):
-//       e = exp2(s c - z), written back in place; l += e.  No separate max pass, no shuffles inside
-//       the pass.  Per tile a 6-shuffle reduce-scatter merges (z, l) over the 4 lanes of a row; shifts
-//       per (thread, row, chunk) (int16) and (z, l) per (row, chunk) go to shared memory; B warps
-//       never wait for anything but the next S half.
-//   C warps (4: one per lane quadrant) — statistics and pass C.  (z, l) of a row are merged over
-//       the four chunks and the CL CTAs with exact power-of-two rescaling built by integer
-//       arithmetic (no MUFU); across CTAs with st.async + a transaction-count mbarrier per
-//       (buffer, quadrant) — no fence, no cluster barrier.  w_(row,chunk) = 2^(z - Z_row) / L_row.
-//       pass C (one TMEM read):  acc_j += sum_i e_ij w_i  in per-thread registers: with the 16x256b
-//       TMEM load shape the column sum over ALL tiles of a segment is a plain packed FFMA2;
-//       lanes are combined once per segment.
+//       read, one write, in the 32x32b shape: a THREAD OWNS A ROW (32 columns per piece, two pieces per
+//       tile), so the maximum, the integer shift z = round(max c) (log2 domain) and the row sum
+//       l = sum 2^(s c - z) are thread-local: no shuffle anywhere in the pass.  e = 2^(s c - z) is written
+//       back in place; (z, l) per (row, 32-column piece) go to shared memory.
+//   S warps (2: two lane quadrants each, lane = row) — statistics.  (z, l) of a row are merged over its
+//       eight pieces and the CL CTAs with exact power-of-two rescaling built by integer arithmetic (no
+//       MUFU); across CTAs with st.async + a transaction-count mbarrier per (buffer, quadrant) — no
+//       fence, no cluster barrier.  The weight of (row, piece), w = 2^(z_piece - Z_row) / L_row, is
+//       written over the piece's (z, l) entry as the pair {w, w}, ready for a packed FFMA2.
+//   C warps (4: one per lane quadrant) — pass C only (one TMEM read, 16x256b shape):
+//       acc_j += sum_i e_ij w_i  in per-thread registers; with that load shape the column sum over ALL
+//       tiles of a segment is a plain packed FFMA2; lanes are combined once per segment.  Each TMEM half
+//       is handed back to the MMA warp as soon as it has been read.
 // TMEM holds two 128 x 256 fp32 S buffers (all 512 columns).  The K panel is double-buffered so a
 // segment change costs no bubble.
 //
 // Warp roles (768 threads): warps 0-15 B (q = warp & 3, cq = warp >> 2), 16-19 C (q = warp & 3),
-// 20 TMA producer, 21 MMA issuer, 22-23 idle (they complete the warpgroup whose registers
-// setmaxnreg hands to the C warps).
+// 20 TMA producer, 21 MMA issuer, 22-23 S (quadrants 2 (warp - 22) + {0, 1}).
 // Output: partial[unit][p][j] (fp32), p = index of the range among those that touch the unit;
 // the select kernel sums the strips in fixed order, so scores are bit-reproducible run to run
 // (no atomics anywhere).
@@ -49,9 +47,10 @@ constexpr int kBWarps = 16;                   // pass B warps: 0..15
 constexpr int kCWarp0 = 16;                   // pass C warps: 16..19
 constexpr int kProducerWarp = 20;
 constexpr int kMmaWarp = 21;
-constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works per warpgroup); warps 22, 23 idle
+constexpr int kStatWarp0 = 22;                // statistics warps: 22, 23
+constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works per warpgroup)
 // registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
-// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, idle) = 6 x 80
+// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, statistics) = 6 x 80
 constexpr int kRegsB = 72, kRegsC = 152, kRegsOther = 40;
 thread_local char g_tc_err[256] = "";
 
@@ -68,12 +67,12 @@ struct Smem {
   static constexpr int kOffK = 0;
   static constexpr int kOffQ = kOffK + kKStages * kKBytes;
   static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 C warps][256]
-  static constexpr int kOffZc = kOffColsum + 4 * kKeysPerCta * 4;        // short [2 bufs][4 q][4 chunks][4 rows][32 lanes] (unbiased shifts)
-  static constexpr int kOffRstat = kOffZc + 2 * 4 * 4 * 4 * 32 * 2;      // uint2 [2 bufs][4 chunks][128 rows]
-  static constexpr int kOffXch = kOffRstat + 2 * 4 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
+  // per (buffer, 32-column piece, row): (z, l) written by the B warps, overwritten by the S warps with {w, w}
+  static constexpr int kOffRstat = kOffColsum + 4 * kKeysPerCta * 4;     // uint2 [2 bufs][8 pieces][128 rows]
+  static constexpr int kOffXch = kOffRstat + 2 * 8 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
   static constexpr int kOffBars = kOffXch + 2 * 4 * CL * 32 * 8;
-  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] = 26 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 26 * 8;
+  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] wbar[2][4] = 34 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 34 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
@@ -116,94 +115,70 @@ __device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long 
 // columns the MMA of half hf produces (0 = half not issued)
 __device__ __forceinline__ int half_cols(int n_cols, int hf) { return min(max(n_cols - kHalf * hf, 0), kHalf); }
 
-// ---- pass B on one piece: 2 rows (K0, K0+1) x 16 columns of chunk CH (of this half) -----------------
-// r[4i+j] = row K0, r[4i+2+j] = row K0+1, column col0 + 8 i + 2 qd + j of the CTA's 256; e gets the
-// exponentials in the same layout.  Online softmax with exact power-of-two rescaling: the shift of
-// this (row, chunk) is the running maximum z = max(z_run, round(m c)) of the thread's integer shifts
-// (log2 domain), so e <= 2^0.5; l_run is rescaled by 2^(z_old - z) built from the exponent field (no
-// MUFU).  Shifts are biased ints (see kZFloor); a fully masked piece has m = -inf -> as_int(t) < 0
-// -> z = floor / z_run, e = 0.
-template <int CH, int K0, bool RAGGED>
-__device__ __forceinline__ void pass_b_body(const uint32_t (&rin)[32], uint32_t (&e)[32], int (&zc)[2][4],
-                                            int (&zrun)[4], float (&lrun)[4], float cs, int qd, int col0,
+// ---- pass B on one piece: ONE row x 32 columns [col0, col0 + 32) of the CTA's 256 -------------------------
+// x[i] = logit of column col0 + i; on return x[i] = e = 2^(s c - z) with the shift z = round(max c) of THIS
+// piece (log2 domain), so e <= 2^0.5, and l = sum e.  Shifts are biased ints (the bit pattern of z + kMagic,
+// see kZFloor); a fully masked piece has max = -inf -> as_int(t) < 0 -> z = floor, e = 0, l = 0.
+template <bool RAGGED>
+__device__ __forceinline__ void pass_b_body(uint32_t (&r)[32], int& z_out, float& l_out, float cs, int col0,
                                             int c_lo, int c_hi) {
   float x[32];
 #pragma unroll
-  for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(rin[i]);
+  for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(r[i]);
   if (RAGGED) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-#pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        const int col = col0 + 8 * i + 2 * qd + j;
-        if (col < c_lo || col >= c_hi) { x[4 * i + j] = __int_as_float(0xff800000); x[4 * i + 2 + j] = __int_as_float(0xff800000); }
-      }
-    }
+    for (int i = 0; i < 32; ++i)
+      if (col0 + i < c_lo || col0 + i >= c_hi) x[i] = __int_as_float(0xff800000);
   }
-  float m0 = max3(x[0], x[1], x[4]), m1 = max3(x[2], x[3], x[6]);
-  float m0b = max3(x[5], x[8], x[9]), m1b = max3(x[7], x[10], x[11]);
-  m0 = max3(m0, x[12], x[13]);   m1 = max3(m1, x[14], x[15]);
-  m0b = max3(m0b, x[16], x[17]); m1b = max3(m1b, x[18], x[19]);
-  m0 = max3(m0, x[20], x[21]);   m1 = max3(m1, x[22], x[23]);
-  m0b = max3(m0b, x[24], x[25]); m1b = max3(m1b, x[26], x[27]);
-  m0 = max3(m0, x[28], x[29]);   m1 = max3(m1, x[30], x[31]);
-  m0 = fmaxf(m0, m0b);           m1 = fmaxf(m1, m1b);
+  float m0 = max3(x[0], x[1], x[2]), m1 = max3(x[3], x[4], x[5]);
+  float m2 = max3(x[6], x[7], x[8]), m3 = max3(x[9], x[10], x[11]);
+  m0 = max3(m0, x[12], x[13]); m1 = max3(m1, x[14], x[15]);
+  m2 = max3(m2, x[16], x[17]); m3 = max3(m3, x[18], x[19]);
+  m0 = max3(m0, x[20], x[21]); m1 = max3(m1, x[22], x[23]);
+  m2 = max3(m2, x[24], x[25]); m3 = max3(m3, x[26], x[27]);
+  m0 = max3(m0, x[28], x[29]); m1 = max3(m1, x[30], x[31]);
+  const float m = fmaxf(max3(m0, m1, m2), m3);
   // t = round(m c) + kMagic as a float; its bit pattern is the biased integer shift
-  const float t0 = fminf(fmaf(m0, cs, kMagic), kMagic + kZLim);
-  const float t1 = fminf(fmaf(m1, cs, kMagic), kMagic + kZLim);
-  int z0, z1;
-  float l0s, l1s;
-  if (CH == 0) {                                 // first chunk of the tile: nothing accumulated yet
-    z0 = max(kZFloor, __float_as_int(t0)); z1 = max(kZFloor, __float_as_int(t1));
-    l0s = 0.f; l1s = 0.f;
-  } else {
-    z0 = max(zrun[K0], __float_as_int(t0)); z1 = max(zrun[K0 + 1], __float_as_int(t1));
-    l0s = lrun[K0] * pow2i(zrun[K0] - z0); l1s = lrun[K0 + 1] * pow2i(zrun[K0 + 1] - z1);
-  }
-  zrun[K0] = z0; zrun[K0 + 1] = z1;
-  zc[CH][K0] = z0; zc[CH][K0 + 1] = z1;
-  const float nz0 = kMagic - __int_as_float(z0), nz1 = kMagic - __int_as_float(z1);   // = -z, exact
-  const uint64_t cs2 = pk2(cs, cs), nz0_2 = pk2(nz0, nz0), nz1_2 = pk2(nz1, nz1);
-  uint64_t l0 = pk2(l0s, 0.f), l1 = pk2(l1s, 0.f);
+  const float t = fminf(fmaf(m, cs, kMagic), kMagic + kZLim);
+  const int z = max(kZFloor, __float_as_int(t));
+  const float nz = kMagic - __int_as_float(z);                     // = -z, exact
+  const uint64_t cs2 = pk2(cs, cs), nz2 = pk2(nz, nz);
+  uint64_t la = pk2(0.f, 0.f), lb = pk2(0.f, 0.f);
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    // kPolyMask: column groups whose exponentials run on the FMA pipe (never on a ragged chunk,
-    // where masked columns must come out as exact zeros)
-    const bool poly = !RAGGED && ((kPolyMask >> i) & 1);
+  for (int i = 0; i < 16; ++i) {
+    // kPolyMask: column pairs whose exponentials run on the FMA pipe (never on a ragged piece, where masked
+    // columns must come out as exact zeros)
+    const bool poly = !RAGGED && ((kPolyMask >> (i & 7)) & 1);
     float a, b;
-    if (poly) exp2_poly2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b);
-    else { upk2(fma2(pk2(x[4 * i], x[4 * i + 1]), cs2, nz0_2), a, b); a = ex2(a); b = ex2(b); }
-    l0 = add2(l0, pk2(a, b));
-    e[4 * i] = __float_as_uint(a); e[4 * i + 1] = __float_as_uint(b);
-    if (poly) exp2_poly2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b);
-    else { upk2(fma2(pk2(x[4 * i + 2], x[4 * i + 3]), cs2, nz1_2), a, b); a = ex2(a); b = ex2(b); }
-    l1 = add2(l1, pk2(a, b));
-    e[4 * i + 2] = __float_as_uint(a); e[4 * i + 3] = __float_as_uint(b);
+    if (poly) exp2_poly2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b);
+    else { upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b); a = ex2(a); b = ex2(b); }
+    if (i & 1) lb = add2(lb, pk2(a, b)); else la = add2(la, pk2(a, b));
+    r[2 * i] = __float_as_uint(a); r[2 * i + 1] = __float_as_uint(b);
   }
   float a, b;
-  upk2(l0, a, b); lrun[K0] = a + b;
-  upk2(l1, a, b); lrun[K0 + 1] = a + b;
+  upk2(add2(la, lb), a, b);
+  z_out = z;
+  l_out = a + b;
 }
-// two copies of the body, so that the common (no ragged edge) path carries no select and no register copies
-template <int CH, int K0>
-__device__ __forceinline__ void pass_b_piece(const uint32_t (&rin)[32], uint32_t (&e)[32], int (&zc)[2][4],
-                                             int (&zrun)[4], float (&lrun)[4], float cs, int qd, int col0,
-                                             int c_lo, int c_hi) {
-  if (col0 >= c_lo && col0 + 64 <= c_hi)        // warp-uniform: false only on the ragged first / last chunk
-    pass_b_body<CH, K0, false>(rin, e, zc, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+// two copies of the body, so that the common (no ragged edge) path carries no select
+__device__ __forceinline__ void pass_b_piece(uint32_t (&r)[32], int& z, float& l, float cs, int col0, int c_lo, int c_hi) {
+  if (col0 >= c_lo && col0 + 32 <= c_hi)        // warp-uniform: false only on a ragged first / last piece
+    pass_b_body<false>(r, z, l, cs, col0, c_lo, c_hi);
   else
-    pass_b_body<CH, K0, true>(rin, e, zc, zrun, lrun, cs, qd, col0, c_lo, c_hi);
+    pass_b_body<true>(r, z, l, cs, col0, c_lo, c_hi);
 }
 
-// ---- pass C on one piece: acc[C*8 + i] (columns 64 C + 8i+2qd+{0,1}) += e(row) * w(row, chunk) -------
-template <int C, int K0>
-__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[32], const float (&w)[4][4]) {
-  const uint64_t w0 = pk2(w[C][K0], w[C][K0]), w1 = pk2(w[C][K0 + 1], w[C][K0 + 1]);
+// ---- pass C on one loaded piece (16 rows x 64 columns of chunk C): acc[C*8 + i] (columns 64 C + 8i+2qd+{0,1})
+// += e(row) * w(row, 32-column piece).  r[4i+{0,1}] = row lr (+16 for the upper lanes), r[4i+{2,3}] = that row + 8;
+// w?a = {w, w} of the chunk's first 32-column piece, w?b of its second.
+template <int C>
+__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[32], uint64_t w0a, uint64_t w1a,
+                                             uint64_t w0b, uint64_t w1b) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     uint64_t a = acc[C * 8 + i];
-    a = fma2(pk2u(r[4 * i], r[4 * i + 1]), w0, a);
-    a = fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), w1, a);
+    a = fma2(pk2u(r[4 * i], r[4 * i + 1]), i < 4 ? w0a : w0b, a);
+    a = fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), i < 4 ? w1a : w1b, a);
     acc[C * 8 + i] = a;
   }
 }
@@ -224,12 +199,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t sK = base + SM::kOffK;
   const uint32_t sQ = base + SM::kOffQ;
   float* colsum = reinterpret_cast<float*>(gbase + SM::kOffColsum);
-  short* zcs = reinterpret_cast<short*>(gbase + SM::kOffZc);
   uint2* rstat = reinterpret_cast<uint2*>(gbase + SM::kOffRstat);
   uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
   const uint32_t qfull = bars, qempty = bars + 16, kfull = bars + 32, kempty = bars + 48;
-  const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144;
+  const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144, wbar = bars + 208;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform for the compiler
@@ -246,6 +220,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     }
     for (int i = 0; i < 2; ++i) mbar_init(bdone + 8 * i, kBWarps);  // one arrive per B warp
     for (int i = 0; i < 8; ++i) mbar_init(xbar + 8 * i, 1);        // per (buffer, quadrant)
+    for (int i = 0; i < 8; ++i) mbar_init(wbar + 8 * i, 1);        // per (buffer, quadrant): weights ready
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
@@ -384,6 +359,80 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         }
       }
     }
+  } else {
+    // ================================ S warps: row statistics -> weights =============================
+    // Each of the two warps serves two lane quadrants (lane = row).  Nothing here touches TMEM: the warps read
+    // the (z, l) the B warps left per (row, piece), merge them over the row (and the cluster), and overwrite
+    // each entry with the pair {w, w}, w = 2^(z_piece - Z_row) / L_row.
+    const int q0 = 2 * (warp - kStatWarp0);
+    int tile_iter = 0;
+    for (long long g = g_begin; g < g_end;) {
+      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
+      g += it.t1 - it.t0;
+      if (!it.ok) continue;
+      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
+        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
+        mbar_wait(bdone + 8 * b, par);
+        int zq[2];
+        float lq[2];
+#pragma unroll
+        for (int qq = 0; qq < 2; ++qq) {
+          const int q = q0 + qq;
+          uint2 sc[8];
+#pragma unroll
+          for (int pc = 0; pc < 8; ++pc) sc[pc] = rstat[(b * 8 + pc) * 128 + q * 32 + lane];
+          int z_row = max(max(max((int)sc[0].x, (int)sc[1].x), max((int)sc[2].x, (int)sc[3].x)),
+                          max(max((int)sc[4].x, (int)sc[5].x), max((int)sc[6].x, (int)sc[7].x)));
+          float l_row = 0.f;
+#pragma unroll
+          for (int pc = 0; pc < 8; ++pc) l_row += __uint_as_float(sc[pc].y) * pow2i((int)sc[pc].x - z_row);
+          if (CL > 1) {
+            // lane publishes its row to every peer CTA
+            const uint32_t bar = xbar + 8 * (b * 4 + q);
+            uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
+            if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
+            __syncwarp();
+            const uint32_t la = smem_u32(slot + rank * 32 + lane);
+#pragma unroll
+            for (int pr = 0; pr < CL; ++pr)
+              if (pr != rank) st_async_b32x2(mapa(la, pr), (uint32_t)z_row, __float_as_uint(l_row), mapa(bar, pr));
+          }
+          zq[qq] = z_row; lq[qq] = l_row;
+        }
+#pragma unroll
+        for (int qq = 0; qq < 2; ++qq) {
+          const int q = q0 + qq;
+          int z_row = zq[qq];
+          float l_row = lq[qq];
+          if (CL > 1) {
+            // merge the row over the CTAs in rank order (identical bits on every CTA)
+            const uint32_t bar = xbar + 8 * (b * 4 + q);
+            const uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
+            mbar_wait(bar, par);
+            int Z = z_row;
+#pragma unroll
+            for (int pr = 0; pr < CL; ++pr) if (pr != rank) Z = max(Z, (int)slot[pr * 32 + lane].x);
+            float L = 0.f;
+#pragma unroll
+            for (int pr = 0; pr < CL; ++pr) {
+              const uint2 v = slot[pr * 32 + lane];
+              L += (pr == rank) ? l_row * pow2i(z_row - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
+            }
+            z_row = Z; l_row = L;
+          }
+          const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + q * 32 + lane;
+          const float inv_row = (l_row > 0.f && tok < c.W) ? __fdividef(1.f, l_row) : 0.f;   // rows past the window contribute nothing
+#pragma unroll
+          for (int pc = 0; pc < 8; ++pc) {
+            uint2* e = rstat + (b * 8 + pc) * 128 + q * 32 + lane;
+            const uint32_t w = __float_as_uint(inv_row * pow2i((int)e->x - z_row));
+            *e = make_uint2(w, w);
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(wbar + 8 * (b * 4 + q));      // release: the C warp of this quadrant may read the weights
+        }
+      }
+    }
   }
   } else if (warp >= kCWarp0) {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(kRegsC));
@@ -407,92 +456,58 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       const int n_chunks = (it.n_cols + 63) >> 6;                       // 1 .. 4
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        mbar_wait(bdone + 8 * b, par);
-        // ---- row statistics (lane = row of this quadrant): two halves -> CTA -> cluster ----
-        int z_row;
-        float l_row;
-        {
-          uint2 sc[4];
-#pragma unroll
-          for (int ch = 0; ch < 4; ++ch) sc[ch] = rstat[(b * 4 + ch) * 128 + q * 32 + lane];
-          z_row = max(max((int)sc[0].x, (int)sc[1].x), max((int)sc[2].x, (int)sc[3].x));
-          l_row = 0.f;
-#pragma unroll
-          for (int ch = 0; ch < 4; ++ch) l_row += __uint_as_float(sc[ch].y) * pow2i((int)sc[ch].x - z_row);
-        }
-        if (CL > 1) {
-          // lane publishes its row to every peer CTA ...
-          const uint32_t bar = xbar + 8 * (b * 4 + q);
-          uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
-          if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
-          __syncwarp();
-          const uint32_t la = smem_u32(slot + rank * 32 + lane);
-#pragma unroll
-          for (int p = 0; p < CL; ++p)
-            if (p != rank) st_async_b32x2(mapa(la, p), (uint32_t)z_row, __float_as_uint(l_row), mapa(bar, p));
-          mbar_wait(bar, par);
-          // ... and merges that row over the CTAs in rank order (identical bits on every CTA)
-          int Z = z_row;
-#pragma unroll
-          for (int p = 0; p < CL; ++p) if (p != rank) Z = max(Z, (int)slot[p * 32 + lane].x);
-          float L = 0.f;
-#pragma unroll
-          for (int p = 0; p < CL; ++p) {
-            const uint2 v = slot[p * 32 + lane];
-            L += (p == rank) ? l_row * pow2i(z_row - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
-          }
-          z_row = Z; l_row = L;
-        }
-        const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + q * 32 + lane;
-        const float inv_row = (l_row > 0.f && tok < c.W) ? __fdividef(1.f, l_row) : 0.f;   // rows past the window contribute nothing
-        float w[4][4];
-        {
-          const short* zt = zcs + (size_t)((b * 4 + q) * 16) * 32 + lane;
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const int zf = __shfl_sync(0xffffffffu, z_row, lr + 8 * k) - kMagicBits;
-            const float iv = __shfl_sync(0xffffffffu, inv_row, lr + 8 * k);
-#pragma unroll
-            for (int ch = 0; ch < 4; ++ch)
-              w[ch][k] = ch < n_chunks ? iv * pow2i(zt[(ch * 4 + k) * 32] - zf) : 0.f;
-          }
-        }
-        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
+        mbar_wait(wbar + 8 * (b * 4 + q), par);             // the S warp has the weights of this quadrant's rows ready
+        // (which implies bdone: every B warp has written its e back; the barrier chain carries the ordering)
         tc_fence_after();
+        // weights: rows lr + 8k (k = 0..3) x pieces 0..7, {w, w} pairs, fetched just before their use
+        const uint2* wrow = rstat + (size_t)(b * 8) * 128 + q * 32 + lr;
+        auto wld = [&](int pc, int k) -> uint64_t {
+          const uint2 v = wrow[pc * 128 + 8 * k];
+          return pk2u(v.x, v.y);
+        };
+        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
         const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
         uint32_t ra[32], rb[32];
         tmem_ld_16x256b_x8(ta, ra);
+        uint64_t w0a = wld(0, 0), w1a = wld(0, 1), w0b = wld(1, 0), w1b = wld(1, 1);
+        uint64_t v0a = wld(0, 2), v1a = wld(0, 3), v0b = wld(1, 2), v1b = wld(1, 3);
         tmem_wait_ld();
         tmem_ld_16x256b_x8(ta_hi, rb);
-        pass_c_piece<0, 0>(ra, acc, w);
+        pass_c_piece<0>(ra, acc, w0a, w1a, w0b, w1b);
         tmem_wait_ld();
         if (n_chunks > 1) tmem_ld_16x256b_x8(ta + 64, ra);
-        pass_c_piece<0, 2>(rb, acc, w);
+        pass_c_piece<0>(rb, acc, v0a, v1a, v0b, v1b);
         if (n_chunks > 1) {
+          w0a = wld(2, 0); w1a = wld(2, 1); w0b = wld(3, 0); w1b = wld(3, 1);
+          v0a = wld(2, 2); v1a = wld(2, 3); v0b = wld(3, 2); v1b = wld(3, 3);
           tmem_wait_ld();
           tmem_ld_16x256b_x8(ta_hi + 64, rb);
-          pass_c_piece<1, 0>(ra, acc, w);
+          pass_c_piece<1>(ra, acc, w0a, w1a, w0b, w1b);
           tmem_wait_ld();
           if (n_chunks > 2) tmem_ld_16x256b_x8(ta + 128, ra);
-          pass_c_piece<1, 2>(rb, acc, w);
+          pass_c_piece<1>(rb, acc, v0a, v1a, v0b, v1b);
         }
         // half 0 has been read completely: the MMA may refill it
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 0));
         if (n_chunks > 2) {
+          w0a = wld(4, 0); w1a = wld(4, 1); w0b = wld(5, 0); w1b = wld(5, 1);
+          v0a = wld(4, 2); v1a = wld(4, 3); v0b = wld(5, 2); v1b = wld(5, 3);
           tmem_wait_ld();
           tmem_ld_16x256b_x8(ta_hi + 128, rb);
-          pass_c_piece<2, 0>(ra, acc, w);
+          pass_c_piece<2>(ra, acc, w0a, w1a, w0b, w1b);
           tmem_wait_ld();
           if (n_chunks > 3) tmem_ld_16x256b_x8(ta + 192, ra);
-          pass_c_piece<2, 2>(rb, acc, w);
+          pass_c_piece<2>(rb, acc, v0a, v1a, v0b, v1b);
           if (n_chunks > 3) {
+            w0a = wld(6, 0); w1a = wld(6, 1); w0b = wld(7, 0); w1b = wld(7, 1);
+            v0a = wld(6, 2); v1a = wld(6, 3); v0b = wld(7, 2); v1b = wld(7, 3);
             tmem_wait_ld();
             tmem_ld_16x256b_x8(ta_hi + 192, rb);
-            pass_c_piece<3, 0>(ra, acc, w);
+            pass_c_piece<3>(ra, acc, w0a, w1a, w0b, w1b);
             tmem_wait_ld();
-            pass_c_piece<3, 2>(rb, acc, w);
+            pass_c_piece<3>(rb, acc, v0a, v1a, v0b, v1b);
           }
         }
         tc_fence_before();
@@ -527,7 +542,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     // ================================ B warps: pass B ================================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsB));
     const int q = warp & 3, cq = warp >> 2, hf = cq >> 1;   // TMEM lane quadrant; 64-column chunk; MMA half of the chunk
-    const int qd = lane & 3, lr = lane >> 2;
     const float cs = kLog2e * rsqrtf((float)D);
     const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 64;
     int tile_iter = 0;
@@ -539,55 +553,25 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       const int c_lo = it.c_lo, c_hi = it.c_hi;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        int zc[2][4], zq[4];
-        float lq[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { zq[k] = kZFloor; lq[k] = 0.f; zc[0][k] = kZFloor; }
+        int z0 = kZFloor, z1 = kZFloor;
+        float l0 = 0.f, l1 = 0.f;
         mbar_wait(tfull + 8 * (b * 2 + hf), par);
         tc_fence_after();
         if (active) {
-          // ---- pass B: e = 2^(s c - z) in place; z per (thread, row), (z, l) per row ----
-          const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
-          uint32_t ra[32], rb[32], e[32];
-          tmem_ld_16x256b_x8(ta, ra);
+          // ---- pass B: e = 2^(s c - z) in place; (z, l) per (row, piece); the thread owns row 32 q + lane ----
+          const uint32_t ta = tq + b * kKeysPerCta;
+          uint32_t ra[32], rb[32];
+          tmem_ld_32x32b_x32(ta, ra);
           tmem_wait_ld();
-          tmem_ld_16x256b_x8(ta_hi, rb);
-          pass_b_piece<0, 0>(ra, e, zc, zq, lq, cs, qd, cq * 64, c_lo, c_hi);
-          tmem_st_16x256b_x8(ta, e);
+          tmem_ld_32x32b_x32(ta + 32, rb);
+          pass_b_piece(ra, z0, l0, cs, cq * 64, c_lo, c_hi);
+          tmem_st_32x32b_x32(ta, ra);
           tmem_wait_ld();
-          pass_b_piece<0, 2>(rb, e, zc, zq, lq, cs, qd, cq * 64, c_lo, c_hi);
-          tmem_st_16x256b_x8(ta_hi, e);
+          pass_b_piece(rb, z1, l1, cs, cq * 64 + 32, c_lo, c_hi);
+          tmem_st_32x32b_x32(ta + 32, rb);
         }
-        // ---- row statistics of this chunk: quad -> row; shifts and (z, l) to shared memory ----
-        {
-          short* zt = zcs + (size_t)((b * 4 + q) * 16 + cq * 4) * 32 + lane;
-#pragma unroll
-          for (int k = 0; k < 4; ++k) zt[k * 32] = (short)(zc[0][k] - kMagicBits);
-        }
-        // reduce-scatter over the 4 lanes of a quad: lane qd ends up with row k = qd (6 shuffles)
-        int z_row;
-        float l_row;
-        {
-          const bool p1 = qd & 1, p2 = qd & 2;
-          // step 1 (lane ^ 1): keep rows {p1, p1 + 2}, hand the other two over
-          const int ks0 = p1 ? zq[1] : zq[0], ks1 = p1 ? zq[3] : zq[2];
-          const float kl0 = p1 ? lq[1] : lq[0], kl1 = p1 ? lq[3] : lq[2];
-          const int rz0 = __shfl_xor_sync(0xffffffffu, p1 ? zq[0] : zq[1], 1);
-          const int rz1 = __shfl_xor_sync(0xffffffffu, p1 ? zq[2] : zq[3], 1);
-          const float rl0 = __shfl_xor_sync(0xffffffffu, p1 ? lq[0] : lq[1], 1);
-          const float rl1 = __shfl_xor_sync(0xffffffffu, p1 ? lq[2] : lq[3], 1);
-          const int za = max(ks0, rz0), zb = max(ks1, rz1);
-          const float la = kl0 * pow2i(ks0 - za) + rl0 * pow2i(rz0 - za);
-          const float lb = kl1 * pow2i(ks1 - zb) + rl1 * pow2i(rz1 - zb);
-          // step 2 (lane ^ 2): keep row p1 + 2 p2 = qd
-          const int kz = p2 ? zb : za;
-          const float kl = p2 ? lb : la;
-          const int rz = __shfl_xor_sync(0xffffffffu, p2 ? za : zb, 2);
-          const float rl = __shfl_xor_sync(0xffffffffu, p2 ? la : lb, 2);
-          z_row = max(kz, rz);
-          l_row = kl * pow2i(kz - z_row) + rl * pow2i(rz - z_row);
-        }
-        rstat[(b * 4 + cq) * 128 + q * 32 + lr + 8 * qd] = make_uint2((uint32_t)z_row, __float_as_uint(l_row));
+        rstat[(b * 8 + 2 * cq) * 128 + q * 32 + lane] = make_uint2((uint32_t)z0, __float_as_uint(l0));
+        rstat[(b * 8 + 2 * cq + 1) * 128 + q * 32 + lane] = make_uint2((uint32_t)z1, __float_as_uint(l1));
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
