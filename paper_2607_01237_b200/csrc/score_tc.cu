@@ -14,26 +14,28 @@
 //   S[128 x 256] = Q_tile[128 x d] . K_cta[256 x d]^T      tcgen05.mma kind::f16, bf16 in, fp32 in TMEM,
 //       issued as two N <= 128 halves, each with its own full / empty barrier, so a half is
 //       refilled as soon as its column sums have been taken.
-//   The softmax is split over SPECIALISED warps, none of which waits for more than one thing:
-//   B warps (16: TMEM lane quadrant q x 64-column chunk cq) — pass B, the only MUFU work.  One TMEM
-//       read, one write, in the 32x32b shape: a THREAD OWNS A ROW (32 columns per piece, two pieces per
-//       tile), so the maximum, the integer shift z = round(max c) (log2 domain) and the row sum
+//   The softmax is split over SPECIALISED warps:
+//   B warps (16: TMEM lane quadrant q x 32-column piece cq of each MMA half) — pass B, the only MUFU work.
+//       One TMEM read, one write, in the 32x32b shape: a THREAD OWNS A ROW (32 columns per piece, one piece per
+//       half), so the maximum, the integer shift z = round(max c) (log2 domain) and the row sum
 //       l = sum 2^(s c - z) are thread-local: no shuffle anywhere in the pass.  e = 2^(s c - z) is written
 //       back in place; (z, l) per (row, 32-column piece) go to shared memory.
-//   S warps (2: two lane quadrants each, lane = row) — statistics.  (z, l) of a row are merged over its
-//       eight pieces and the CL CTAs with exact power-of-two rescaling built by integer arithmetic (no
-//       MUFU); across CTAs with st.async + a transaction-count mbarrier per (buffer, quadrant) — no
-//       fence, no cluster barrier.  The weight of (row, piece), w = 2^(z_piece - Z_row) / L_row, is
-//       written over the piece's (z, l) entry as the pair {w, w}, ready for a packed FFMA2.
-//   C warps (4: one per lane quadrant) — pass C only (one TMEM read, 16x256b shape):
-//       acc_j += sum_i e_ij w_i  in per-thread registers; with that load shape the column sum over ALL
-//       tiles of a segment is a plain packed FFMA2; lanes are combined once per segment.  Each TMEM half
-//       is handed back to the MMA warp as soon as it has been read.
+//   C warps (4: one per lane quadrant) — statistics, then pass C.  With lane = row, (z, l) of a row are merged
+//       over its eight pieces and the CL CTAs with exact power-of-two rescaling built by integer arithmetic
+//       (no MUFU); across CTAs with st.async + a transaction-count mbarrier per (buffer, quadrant) — no
+//       fence, no cluster barrier.  The weight of (row, piece), w = 2^(z_piece - Z_row) / L_row, goes over
+//       the piece's (z, l) entry as the pair {w, w}, ready for a packed FFMA2 (the four warps work on their
+//       own quadrants in parallel: their shared-memory and MUFU.RCP operations queue behind the B warps'
+//       exponentials, so the count of such operations per warp is what this step costs).  Pass C (one TMEM
+//       read, 16x256b shape): acc_j += sum_i e_ij w_i in per-thread registers; with that load shape the
+//       column sum over ALL tiles of a segment is a plain packed FFMA2; lanes are combined once per
+//       segment.  Each TMEM half is handed back to the MMA warp as soon as it has been read.
 // TMEM holds two 128 x 256 fp32 S buffers (all 512 columns).  The K panel is double-buffered so a
 // segment change costs no bubble.
 //
-// Warp roles (768 threads): warps 0-15 B (q = warp & 3, cq = warp >> 2), 16-19 C (q = warp & 3),
-// 20 TMA producer, 21 MMA issuer, 22-23 S (quadrants 2 (warp - 22) + {0, 1}).
+// Warp roles (768 threads): warps 0-15 B (q = warp & 3, piece cq = warp >> 2 of each MMA half), 16-19 C (q = warp & 3),
+// 20 TMA producer, 21 MMA issuer, 22-23 idle (they complete the warpgroup whose registers setmaxnreg hands to
+// the C warps).
 // Output: partial[unit][p][j] (fp32), p = index of the range among those that touch the unit;
 // the select kernel sums the strips in fixed order, so scores are bit-reproducible run to run
 // (no atomics anywhere).
@@ -47,12 +49,24 @@ constexpr int kBWarps = 16;                   // pass B warps: 0..15
 constexpr int kCWarp0 = 16;                   // pass C warps: 16..19
 constexpr int kProducerWarp = 20;
 constexpr int kMmaWarp = 21;
-constexpr int kStatWarp0 = 22;                // statistics warps: 22, 23
 constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works per warpgroup)
 // registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
-// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, statistics) = 6 x 80
+// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, idle) = 6 x 80
 constexpr int kRegsB = 72, kRegsC = 152, kRegsOther = 40;
 thread_local char g_tc_err[256] = "";
+
+#ifndef KARA_B_PREFETCH
+#define KARA_B_PREFETCH 0                      // 1: the TMEM load of a tile's second piece is issued before the exponentials of the first
+#endif
+#ifdef KARA_TC_TRACE
+// debug build: clock64() stamps of CTA 0's warp roles per tile (see kara_tc_trace_read below)
+constexpr int kTraceTiles = 64, kTraceEv = 8, kTraceRoles = 5;   // roles: 0 = B warp 0, 1 = B warp 15, 2 = MMA, 3 = C warp 16, 4 = C warp 17
+__device__ long long g_trace[kTraceRoles * kTraceTiles * kTraceEv];
+#define KARA_TRACE(role, ti, ev)                                                                     \
+  do { if (blockIdx.x == 0 && lane == 0 && (ti) < kTraceTiles) g_trace[((role) * kTraceTiles + (ti)) * kTraceEv + (ev)] = clock64(); } while (0)
+#else
+#define KARA_TRACE(role, ti, ev) do { } while (0)
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // shared-memory carve-up (dynamic smem, manually aligned to 1024 B for the 128B swizzle)
@@ -67,12 +81,13 @@ struct Smem {
   static constexpr int kOffK = 0;
   static constexpr int kOffQ = kOffK + kKStages * kKBytes;
   static constexpr int kOffColsum = kOffQ + kQStages * kQStageBytes;     // float [4 C warps][256]
-  // per (buffer, 32-column piece, row): (z, l) written by the B warps, overwritten by the S warps with {w, w}
-  static constexpr int kOffRstat = kOffColsum + 4 * kKeysPerCta * 4;     // uint2 [2 bufs][8 pieces][128 rows]
-  static constexpr int kOffXch = kOffRstat + 2 * 8 * 128 * 8;            // uint2 [2 bufs][4 q][CL][32]
+  // per (buffer, piece column cq, row): {z, l} of the row's piece cq in half 0 and in half 1, written by the B warps,
+  // overwritten by the C warps with the weight pairs {w0, w0, w1, w1}
+  static constexpr int kOffRstat = kOffColsum + 4 * kKeysPerCta * 4;     // uint4 [2 bufs][4 cq][128 rows]
+  static constexpr int kOffXch = kOffRstat + 2 * 4 * 128 * 16;           // uint2 [2 bufs][4 q][CL][32]
   static constexpr int kOffBars = kOffXch + 2 * 4 * CL * 32 * 8;
-  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] wbar[2][4] = 34 x 8 B
-  static constexpr int kOffTmemPtr = kOffBars + 34 * 8;
+  // barriers: qfull[2] qempty[2] kfull[2] kempty[2] tfull[2][2] tempty[2][2] bdone[2] xbar[2][4] = 26 x 8 B
+  static constexpr int kOffTmemPtr = kOffBars + 26 * 8;
   static constexpr int kBytes = kOffTmemPtr + 16;
   static constexpr int kAlloc = kBytes + 1024;   // slack for manual alignment
 };
@@ -151,7 +166,11 @@ __device__ __forceinline__ void pass_b_body(uint32_t (&r)[32], int& z_out, float
     const bool poly = !RAGGED && ((kPolyMask >> (i & 7)) & 1);
     float a, b;
     if (poly) exp2_poly2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b);
+#ifdef KARA_DBG_NO_EX2
+    else { upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b); }
+#else
     else { upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b); a = ex2(a); b = ex2(b); }
+#endif
     if (i & 1) lb = add2(lb, pk2(a, b)); else la = add2(la, pk2(a, b));
     r[2 * i] = __float_as_uint(a); r[2 * i + 1] = __float_as_uint(b);
   }
@@ -199,11 +218,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   const uint32_t sK = base + SM::kOffK;
   const uint32_t sQ = base + SM::kOffQ;
   float* colsum = reinterpret_cast<float*>(gbase + SM::kOffColsum);
-  uint2* rstat = reinterpret_cast<uint2*>(gbase + SM::kOffRstat);
+  uint4* rstat = reinterpret_cast<uint4*>(gbase + SM::kOffRstat);
   uint2* xch = reinterpret_cast<uint2*>(gbase + SM::kOffXch);
   const uint32_t bars = base + SM::kOffBars;
   const uint32_t qfull = bars, qempty = bars + 16, kfull = bars + 32, kempty = bars + 48;
-  const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144, wbar = bars + 208;
+  const uint32_t tfull = bars + 64, tempty = bars + 96, bdone = bars + 128, xbar = bars + 144;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + SM::kOffTmemPtr);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;   // warp-uniform for the compiler
@@ -218,9 +237,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     for (int i = 0; i < 4; ++i) {
       mbar_init(tfull + 8 * i, 1); mbar_init(tempty + 8 * i, 4);   // one arrive per C warp
     }
-    for (int i = 0; i < 2; ++i) mbar_init(bdone + 8 * i, kBWarps);  // one arrive per B warp
+    for (int i = 0; i < 2; ++i) mbar_init(bdone + 8 * i, kBWarps);  // one arrive per B warp; all four C warps wait on it
     for (int i = 0; i < 8; ++i) mbar_init(xbar + 8 * i, 1);        // per (buffer, quadrant)
-    for (int i = 0; i < 8; ++i) mbar_init(wbar + 8 * i, 1);        // per (buffer, quadrant): weights ready
     fence_barrier_init();
   }
   if (warp == kMmaWarp) tmem_alloc(smem_u32((const void*)tmem_ptr), kTmemCols);
@@ -327,12 +345,15 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       for (int i = 0; i < n_tiles; ++i, ++q_iter, ++tile_iter) {
         const int stage = q_iter % QS, quse = q_iter / QS;
         const int buf = tile_iter & 1, tuse = tile_iter >> 1;
+        KARA_TRACE(2, tile_iter, 0);
         mbar_wait(qfull + 8 * stage, quse & 1);
+        KARA_TRACE(2, tile_iter, 1);
         const uint32_t a_lo = ((sQ + stage * SM::kQStageBytes) >> 4) | kDescLo;
 #pragma unroll
         for (int hf = 0; hf < 2; ++hf) {
           mbar_wait(tempty + 8 * (buf * 2 + hf), (tuse & 1) ^ 1);
           tc_fence_after();
+          KARA_TRACE(2, tile_iter, 2 + 2 * hf);
           if (elect_one()) {
             const int nc = half_cols(n_cols, hf);
             if (nc > 0) {
@@ -356,80 +377,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
             }
           }
           __syncwarp();
-        }
-      }
-    }
-  } else {
-    // ================================ S warps: row statistics -> weights =============================
-    // Each of the two warps serves two lane quadrants (lane = row).  Nothing here touches TMEM: the warps read
-    // the (z, l) the B warps left per (row, piece), merge them over the row (and the cluster), and overwrite
-    // each entry with the pair {w, w}, w = 2^(z_piece - Z_row) / L_row.
-    const int q0 = 2 * (warp - kStatWarp0);
-    int tile_iter = 0;
-    for (long long g = g_begin; g < g_end;) {
-      const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
-      g += it.t1 - it.t0;
-      if (!it.ok) continue;
-      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
-        const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        mbar_wait(bdone + 8 * b, par);
-        int zq[2];
-        float lq[2];
-#pragma unroll
-        for (int qq = 0; qq < 2; ++qq) {
-          const int q = q0 + qq;
-          uint2 sc[8];
-#pragma unroll
-          for (int pc = 0; pc < 8; ++pc) sc[pc] = rstat[(b * 8 + pc) * 128 + q * 32 + lane];
-          int z_row = max(max(max((int)sc[0].x, (int)sc[1].x), max((int)sc[2].x, (int)sc[3].x)),
-                          max(max((int)sc[4].x, (int)sc[5].x), max((int)sc[6].x, (int)sc[7].x)));
-          float l_row = 0.f;
-#pragma unroll
-          for (int pc = 0; pc < 8; ++pc) l_row += __uint_as_float(sc[pc].y) * pow2i((int)sc[pc].x - z_row);
-          if (CL > 1) {
-            // lane publishes its row to every peer CTA
-            const uint32_t bar = xbar + 8 * (b * 4 + q);
-            uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
-            if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
-            __syncwarp();
-            const uint32_t la = smem_u32(slot + rank * 32 + lane);
-#pragma unroll
-            for (int pr = 0; pr < CL; ++pr)
-              if (pr != rank) st_async_b32x2(mapa(la, pr), (uint32_t)z_row, __float_as_uint(l_row), mapa(bar, pr));
-          }
-          zq[qq] = z_row; lq[qq] = l_row;
-        }
-#pragma unroll
-        for (int qq = 0; qq < 2; ++qq) {
-          const int q = q0 + qq;
-          int z_row = zq[qq];
-          float l_row = lq[qq];
-          if (CL > 1) {
-            // merge the row over the CTAs in rank order (identical bits on every CTA)
-            const uint32_t bar = xbar + 8 * (b * 4 + q);
-            const uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
-            mbar_wait(bar, par);
-            int Z = z_row;
-#pragma unroll
-            for (int pr = 0; pr < CL; ++pr) if (pr != rank) Z = max(Z, (int)slot[pr * 32 + lane].x);
-            float L = 0.f;
-#pragma unroll
-            for (int pr = 0; pr < CL; ++pr) {
-              const uint2 v = slot[pr * 32 + lane];
-              L += (pr == rank) ? l_row * pow2i(z_row - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
-            }
-            z_row = Z; l_row = L;
-          }
-          const int tok = c.q_row_begin + (tile % tok_tiles) * kTileM + q * 32 + lane;
-          const float inv_row = (l_row > 0.f && tok < c.W) ? __fdividef(1.f, l_row) : 0.f;   // rows past the window contribute nothing
-#pragma unroll
-          for (int pc = 0; pc < 8; ++pc) {
-            uint2* e = rstat + (b * 8 + pc) * 128 + q * 32 + lane;
-            const uint32_t w = __float_as_uint(inv_row * pow2i((int)e->x - z_row));
-            *e = make_uint2(w, w);
-          }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(wbar + 8 * (b * 4 + q));      // release: the C warp of this quadrant may read the weights
+          KARA_TRACE(2, tile_iter, 3 + 2 * hf);
         }
       }
     }
@@ -454,21 +402,88 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         continue;
       }
       const int n_chunks = (it.n_cols + 63) >> 6;                       // 1 .. 4
-      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
+      int tt = it.t0 % tok_tiles;                                       // token tile of `tile` (kept incrementally: no division per tile)
+      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter, tt = (tt + 1 == tok_tiles ? 0 : tt + 1)) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        mbar_wait(wbar + 8 * (b * 4 + q), par);             // the S warp has the weights of this quadrant's rows ready
-        // (which implies bdone: every B warp has written its e back; the barrier chain carries the ordering)
+        KARA_TRACE(3 + (q == 1), tile_iter, 0);
+        mbar_wait(bdone + 8 * b, par);                      // every B warp has written e back and left (z, l) per (row, piece)
+        KARA_TRACE(3 + (q == 1), tile_iter, 1);
+        // the first TMEM read of pass C is requested now: it lands while the statistics below are merged
         tc_fence_after();
-        // weights: rows lr + 8k (k = 0..3) x pieces 0..7, {w, w} pairs, fetched just before their use
-        const uint2* wrow = rstat + (size_t)(b * 8) * 128 + q * 32 + lr;
-        auto wld = [&](int pc, int k) -> uint64_t {
-          const uint2 v = wrow[pc * 128 + 8 * k];
-          return pk2u(v.x, v.y);
-        };
-        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
         const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
         uint32_t ra[32], rb[32];
         tmem_ld_16x256b_x8(ta, ra);
+        // ---- row statistics of this quadrant (lane = row): 8 pieces -> CTA -> cluster -> weights ----
+        {
+          uint4* ent = rstat + (size_t)(b * 4) * 128 + q * 32 + lane;
+          int zp[8];                                         // zp[2 cq + hf]
+          int z_row;
+          float l_row = 0.f;
+          {
+            uint4 sc[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) sc[x] = ent[x * 128];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) { zp[2 * x] = (int)sc[x].x; zp[2 * x + 1] = (int)sc[x].z; }
+            z_row = max(max(max(zp[0], zp[1]), max(zp[2], zp[3])), max(max(zp[4], zp[5]), max(zp[6], zp[7])));
+#pragma unroll
+            for (int x = 0; x < 4; ++x)
+              l_row += __uint_as_float(sc[x].y) * pow2i(zp[2 * x] - z_row) + __uint_as_float(sc[x].w) * pow2i(zp[2 * x + 1] - z_row);
+          }
+          if (CL > 1) {
+            // lane publishes its row to every peer CTA ...
+            const uint32_t bar = xbar + 8 * (b * 4 + q);
+            uint2* slot = xch + (size_t)(b * 4 + q) * CL * 32;
+            if (lane == 0) mbar_expect_tx(bar, (CL - 1) * 32 * 8);
+            __syncwarp();
+            const uint32_t la = smem_u32(slot + rank * 32 + lane);
+#pragma unroll
+            for (int pr = 0; pr < CL; ++pr)
+              if (pr != rank) st_async_b32x2(mapa(la, pr), (uint32_t)z_row, __float_as_uint(l_row), mapa(bar, pr));
+            KARA_TRACE(3 + (q == 1), tile_iter, 2);
+            mbar_wait(bar, par);
+            KARA_TRACE(3 + (q == 1), tile_iter, 3);
+            // ... and merges that row over the CTAs in rank order (identical bits on every CTA)
+            int Z = z_row;
+#pragma unroll
+            for (int pr = 0; pr < CL; ++pr) if (pr != rank) Z = max(Z, (int)slot[pr * 32 + lane].x);
+            float L = 0.f;
+#pragma unroll
+            for (int pr = 0; pr < CL; ++pr) {
+              const uint2 v = slot[pr * 32 + lane];
+              L += (pr == rank) ? l_row * pow2i(z_row - Z) : __uint_as_float(v.y) * pow2i((int)v.x - Z);
+            }
+            z_row = Z; l_row = L;
+          }
+          const int tok = c.q_row_begin + tt * kTileM + q * 32 + lane;
+          // 1 / L on the FMA pipe (a MUFU.RCP would queue behind the B warps' exponentials): the exponent-flip
+          // estimate (12 % off at most) and three Newton steps, relative error < 1e-7
+          float inv_row = __int_as_float(0x7EF311C7 - __float_as_int(l_row));
+#pragma unroll
+          for (int nr = 0; nr < 3; ++nr) inv_row = inv_row * fmaf(-l_row, inv_row, 2.f);
+          if (!(l_row > 0.f) || tok >= c.W) inv_row = 0.f;   // rows past the window contribute nothing
+          // the weights of (row, piece cq of half 0 / half 1) go over the entry as the pairs {w0, w0, w1, w1}
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const uint32_t w0 = __float_as_uint(inv_row * pow2i(zp[2 * x] - z_row));
+            const uint32_t w1 = __float_as_uint(inv_row * pow2i(zp[2 * x + 1] - z_row));
+            ent[x * 128] = make_uint4(w0, w0, w1, w1);
+          }
+          __syncwarp();
+        }
+        tc_fence_after();
+        KARA_TRACE(3 + (q == 1), tile_iter, 4);
+        // weights: rows lr + 8k (k = 0..3) x pieces 0..7, {w, w} pairs, fetched just before their use
+        const uint2* wrow = reinterpret_cast<const uint2*>(rstat + (size_t)(b * 4) * 128 + q * 32 + lr);
+        auto wld = [&](int pc, int k) -> uint64_t {        // piece pc = 4 hf + cq in column order
+          const uint2 v = wrow[(size_t)((pc & 3) * 128 + 8 * k) * 2 + (pc >> 2)];
+          return pk2u(v.x, v.y);
+        };
+#ifdef KARA_DBG_NO_C
+        if (lane == 0) { mbar_arrive(tempty + 8 * (b * 2 + 0)); mbar_arrive(tempty + 8 * (b * 2 + 1)); }
+        continue;
+#endif
+        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
         uint64_t w0a = wld(0, 0), w1a = wld(0, 1), w0b = wld(1, 0), w1b = wld(1, 1);
         uint64_t v0a = wld(0, 2), v1a = wld(0, 3), v0b = wld(1, 2), v1b = wld(1, 3);
         tmem_wait_ld();
@@ -491,6 +506,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 0));
+        KARA_TRACE(3 + (q == 1), tile_iter, 5);
         if (n_chunks > 2) {
           w0a = wld(4, 0); w1a = wld(4, 1); w0b = wld(5, 0); w1b = wld(5, 1);
           v0a = wld(4, 2); v1a = wld(4, 3); v0b = wld(5, 2); v1b = wld(5, 3);
@@ -513,6 +529,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 1));
+        KARA_TRACE(3 + (q == 1), tile_iter, 6);
       }
 
       // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
@@ -541,41 +558,65 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   } else {
     // ================================ B warps: pass B ================================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsB));
-    const int q = warp & 3, cq = warp >> 2, hf = cq >> 1;   // TMEM lane quadrant; 64-column chunk; MMA half of the chunk
+    // warp (q, cq) owns rows [32 q, 32 q + 32) and, in EACH MMA half, the 32-column piece cq: all 16 warps sweep
+    // half 0, then half 1, so the refill of a half has a whole half-sweep of slack and four warps per scheduler
+    // feed the MUFU pipe at any time
+    const int q = warp & 3, cq = warp >> 2;
     const float cs = kLog2e * rsqrtf((float)D);
-    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 64;
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 32;
     int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
       if (!it.ok) continue;
-      const bool active = cq * 64 < it.n_cols;              // the MMA writes this chunk
       const int c_lo = it.c_lo, c_hi = it.c_hi;
+      const bool act0 = cq * 32 < it.n_cols, act1 = kHalf + cq * 32 < it.n_cols;   // the MMA writes this piece of half 0 / 1
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
+        const uint32_t ta = tq + b * kKeysPerCta;
         int z0 = kZFloor, z1 = kZFloor;
         float l0 = 0.f, l1 = 0.f;
-        mbar_wait(tfull + 8 * (b * 2 + hf), par);
+        const bool trc = (warp == 0 || warp == 15);
+        uint32_t ra[32], rb[32];
+        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 0);
+        mbar_wait(tfull + 8 * (b * 2 + 0), par);
         tc_fence_after();
-        if (active) {
-          // ---- pass B: e = 2^(s c - z) in place; (z, l) per (row, piece); the thread owns row 32 q + lane ----
-          const uint32_t ta = tq + b * kKeysPerCta;
-          uint32_t ra[32], rb[32];
-          tmem_ld_32x32b_x32(ta, ra);
-          tmem_wait_ld();
-          tmem_ld_32x32b_x32(ta + 32, rb);
-          pass_b_piece(ra, z0, l0, cs, cq * 64, c_lo, c_hi);
+        tmem_ld_32x32b_x32(ta, ra);                        // (an inactive piece is loaded too and ignored)
+        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 1);
+        // the TMEM load of piece 1 runs under the exponentials of piece 0 (in the B-bound steady state its S half
+        // has landed long before; a starved B warp loses at most the time between the two MMA halves here)
+#if KARA_B_PREFETCH
+        mbar_wait(tfull + 8 * (b * 2 + 1), par);
+        tc_fence_after();
+        tmem_wait_ld();
+        tmem_ld_32x32b_x32(ta + kHalf, rb);
+#else
+        tmem_wait_ld();
+#endif
+        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 2);
+        // ---- pass B: e = 2^(s c - z) in place; (z, l) of (row, piece); the thread owns row 32 q + lane ----
+        if (act0) {
+          pass_b_piece(ra, z0, l0, cs, cq * 32, c_lo, c_hi);
           tmem_st_32x32b_x32(ta, ra);
-          tmem_wait_ld();
-          pass_b_piece(rb, z1, l1, cs, cq * 64 + 32, c_lo, c_hi);
-          tmem_st_32x32b_x32(ta + 32, rb);
         }
-        rstat[(b * 8 + 2 * cq) * 128 + q * 32 + lane] = make_uint2((uint32_t)z0, __float_as_uint(l0));
-        rstat[(b * 8 + 2 * cq + 1) * 128 + q * 32 + lane] = make_uint2((uint32_t)z1, __float_as_uint(l1));
+#if !KARA_B_PREFETCH
+        mbar_wait(tfull + 8 * (b * 2 + 1), par);
+        tc_fence_after();
+        tmem_ld_32x32b_x32(ta + kHalf, rb);
+#endif
+        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 3);
+        tmem_wait_ld();
+        if (act1) {
+          pass_b_piece(rb, z1, l1, cs, kHalf + cq * 32, c_lo, c_hi);
+          tmem_st_32x32b_x32(ta + kHalf, rb);
+        }
+        rstat[(b * 4 + cq) * 128 + q * 32 + lane] = make_uint4((uint32_t)z0, __float_as_uint(l0), (uint32_t)z1, __float_as_uint(l1));
+        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 4);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bdone + 8 * b);
+        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 5);
       }
     }
   }
@@ -665,6 +706,13 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
 }  // namespace
 
 const char* score_tc_error() { return g_tc_err; }
+
+#ifdef KARA_TC_TRACE
+extern "C" int kara_tc_trace_read(long long* out, int n) {
+  if (n > kTraceRoles * kTraceTiles * kTraceEv) n = kTraceRoles * kTraceTiles * kTraceEv;
+  return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * n);
+}
+#endif
 
 int score_tc_attach(ScoreTcState* s, const Geom& g, void* k_pool) {
   s->ready = false;
