@@ -16,8 +16,8 @@
 //       refilled as soon as its column sums have been taken.
 //   The softmax is split over SPECIALISED warps:
 //   B warps (16: TMEM lane quadrant q x 32-column piece cq of each MMA half) — pass B, the only MUFU work.
-//       One TMEM read, one write, in the 32x32b shape: a THREAD OWNS A ROW (32 columns per piece, one piece per
-//       half), so the maximum, the integer shift z = round(max c) (log2 domain) and the row sum
+//       One TMEM read, one write, in the 16x32bx2 shape: a THREAD OWNS 32 CONSECUTIVE COLUMNS OF ONE ROW (a "piece",
+//       one per half), so the maximum, the integer shift z = round(max c) (log2 domain) and the row sum
 //       l = sum 2^(s c - z) are thread-local: no shuffle anywhere in the pass.  e = 2^(s c - z) is written
 //       back in place; (z, l) per (row, 32-column piece) go to shared memory.
 //   C warps (4: one per lane quadrant) — statistics, then pass C.  With lane = row, (z, l) of a row are merged
@@ -51,12 +51,22 @@ constexpr int kProducerWarp = 20;
 constexpr int kMmaWarp = 21;
 constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works per warpgroup)
 // registers: 768 x 80 at launch; setmaxnreg only moves registers inside that allocation:
-// 4 x 72 (B) + 152 (C) + 40 (producer, MMA, idle) = 6 x 80
-constexpr int kRegsB = 72, kRegsC = 152, kRegsOther = 40;
+// 4 x 80 (B: two 32-register TMEM pieces in flight) + 120 (C: 64 accumulators + two 16-register pieces) + 40 (producer, MMA, idle) = 6 x 80
+constexpr int kRegsB = 80, kRegsC = 120, kRegsOther = 40;
 thread_local char g_tc_err[256] = "";
 
 #ifndef KARA_B_PREFETCH
 #define KARA_B_PREFETCH 0                      // 1: the TMEM load of a tile's second piece is issued before the exponentials of the first
+#endif
+#ifndef KARA_B_SHAPE
+#define KARA_B_SHAPE 0                         // TMEM shape of pass B: 0 = 32x32b (thread = lane), 1 = 16x32bx2 (16 lanes x two 32-column pieces)
+#endif
+#if KARA_B_SHAPE == 0
+#define KARA_B_LD tmem_ld_32x32b_x32
+#define KARA_B_ST tmem_st_32x32b_x32
+#else
+#define KARA_B_LD tmem_ld_16x32bx2_x32
+#define KARA_B_ST tmem_st_16x32bx2_x32
 #endif
 #ifdef KARA_TC_TRACE
 // debug build: clock64() stamps of CTA 0's warp roles per tile (see kara_tc_trace_read below)
@@ -180,25 +190,26 @@ __device__ __forceinline__ void pass_b_body(uint32_t (&r)[32], int& z_out, float
   l_out = a + b;
 }
 // two copies of the body, so that the common (no ragged edge) path carries no select
-__device__ __forceinline__ void pass_b_piece(uint32_t (&r)[32], int& z, float& l, float cs, int col0, int c_lo, int c_hi) {
-  if (col0 >= c_lo && col0 + 32 <= c_hi)        // warp-uniform: false only on a ragged first / last piece
+// [colw, colw + colw_n) = the columns the WARP holds (the branch is warp-uniform), col0 = first of the thread's 32
+__device__ __forceinline__ void pass_b_piece(uint32_t (&r)[32], int& z, float& l, float cs, int colw, int colw_n, int col0,
+                                             int c_lo, int c_hi) {
+  if (colw >= c_lo && colw + colw_n <= c_hi)    // false only on a ragged first / last chunk
     pass_b_body<false>(r, z, l, cs, col0, c_lo, c_hi);
   else
     pass_b_body<true>(r, z, l, cs, col0, c_lo, c_hi);
 }
 
-// ---- pass C on one loaded piece (16 rows x 64 columns of chunk C): acc[C*8 + i] (columns 64 C + 8i+2qd+{0,1})
-// += e(row) * w(row, 32-column piece).  r[4i+{0,1}] = row lr (+16 for the upper lanes), r[4i+{2,3}] = that row + 8;
-// w?a = {w, w} of the chunk's first 32-column piece, w?b of its second.
-template <int C>
-__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[32], uint64_t (&acc)[32], uint64_t w0a, uint64_t w1a,
-                                             uint64_t w0b, uint64_t w1b) {
+// ---- pass C on one loaded piece (16 rows x the 32 columns of piece PC): acc[PC*4 + i] (columns 32 PC + 8i+2qd+{0,1})
+// += e(row) * w(row, piece).  r[4i+{0,1}] = row lr (+16 for the upper lanes), r[4i+{2,3}] = that row + 8; w0 / w1 = {w, w}
+// of those two rows.
+template <int PC>
+__device__ __forceinline__ void pass_c_piece(const uint32_t (&r)[16], uint64_t (&acc)[32], uint64_t w0, uint64_t w1) {
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    uint64_t a = acc[C * 8 + i];
-    a = fma2(pk2u(r[4 * i], r[4 * i + 1]), i < 4 ? w0a : w0b, a);
-    a = fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), i < 4 ? w1a : w1b, a);
-    acc[C * 8 + i] = a;
+  for (int i = 0; i < 4; ++i) {
+    uint64_t a = acc[PC * 4 + i];
+    a = fma2(pk2u(r[4 * i], r[4 * i + 1]), w0, a);
+    a = fma2(pk2u(r[4 * i + 2], r[4 * i + 3]), w1, a);
+    acc[PC * 4 + i] = a;
   }
 }
 
@@ -401,7 +412,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         if (rank == 0) for (int j = threadIdx.x & 127; j < c.n_pad; j += 128) out[j] = 0.f;
         continue;
       }
-      const int n_chunks = (it.n_cols + 63) >> 6;                       // 1 .. 4
+      const int n_pieces = (it.n_cols + 31) >> 5;                       // 1 .. 8
       int tt = it.t0 % tok_tiles;                                       // token tile of `tile` (kept incrementally: no division per tile)
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter, tt = (tt + 1 == tok_tiles ? 0 : tt + 1)) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
@@ -411,8 +422,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         // the first TMEM read of pass C is requested now: it lands while the statistics below are merged
         tc_fence_after();
         const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
-        uint32_t ra[32], rb[32];
-        tmem_ld_16x256b_x8(ta, ra);
+        uint32_t ra[16], rb[16];
+        tmem_ld_16x256b_x4(ta, ra);
         // ---- row statistics of this quadrant (lane = row): 8 pieces -> CTA -> cluster -> weights ----
         {
           uint4* ent = rstat + (size_t)(b * 4) * 128 + q * 32 + lane;
@@ -483,49 +494,26 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         if (lane == 0) { mbar_arrive(tempty + 8 * (b * 2 + 0)); mbar_arrive(tempty + 8 * (b * 2 + 1)); }
         continue;
 #endif
-        // ---- pass C: acc_j += sum_i e_ij w_i ; TMEM loads double buffered; halves released early ----
-        uint64_t w0a = wld(0, 0), w1a = wld(0, 1), w0b = wld(1, 0), w1b = wld(1, 1);
-        uint64_t v0a = wld(0, 2), v1a = wld(0, 3), v0b = wld(1, 2), v1b = wld(1, 3);
-        tmem_wait_ld();
-        tmem_ld_16x256b_x8(ta_hi, rb);
-        pass_c_piece<0>(ra, acc, w0a, w1a, w0b, w1b);
-        tmem_wait_ld();
-        if (n_chunks > 1) tmem_ld_16x256b_x8(ta + 64, ra);
-        pass_c_piece<0>(rb, acc, v0a, v1a, v0b, v1b);
-        if (n_chunks > 1) {
-          w0a = wld(2, 0); w1a = wld(2, 1); w0b = wld(3, 0); w1b = wld(3, 1);
-          v0a = wld(2, 2); v1a = wld(2, 3); v0b = wld(3, 2); v1b = wld(3, 3);
-          tmem_wait_ld();
-          tmem_ld_16x256b_x8(ta_hi + 64, rb);
-          pass_c_piece<1>(ra, acc, w0a, w1a, w0b, w1b);
-          tmem_wait_ld();
-          if (n_chunks > 2) tmem_ld_16x256b_x8(ta + 128, ra);
-          pass_c_piece<1>(rb, acc, v0a, v1a, v0b, v1b);
+        // ---- pass C: acc_j += sum_i e_ij w_i, piece by piece (16 rows x 32 columns per TMEM read, the next read in flight
+        // under the FFMA2s of the current one); each half is handed back to the MMA warp as soon as it has been read ----
+#define KARA_C_STEP(PC)                                                                   \
+        if (PC < n_pieces) {                                                              \
+          const uint64_t w0 = wld(PC, 0), w1 = wld(PC, 1), v0 = wld(PC, 2), v1 = wld(PC, 3); \
+          tmem_wait_ld();                                                                 \
+          tmem_ld_16x256b_x4(ta_hi + 32 * PC, rb);                                        \
+          pass_c_piece<PC>(ra, acc, w0, w1);                                              \
+          tmem_wait_ld();                                                                 \
+          if (PC + 1 < n_pieces) tmem_ld_16x256b_x4(ta + 32 * (PC + 1), ra);              \
+          pass_c_piece<PC>(rb, acc, v0, v1);                                              \
         }
+        KARA_C_STEP(0) KARA_C_STEP(1) KARA_C_STEP(2) KARA_C_STEP(3)
         // half 0 has been read completely: the MMA may refill it
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 0));
         KARA_TRACE(3 + (q == 1), tile_iter, 5);
-        if (n_chunks > 2) {
-          w0a = wld(4, 0); w1a = wld(4, 1); w0b = wld(5, 0); w1b = wld(5, 1);
-          v0a = wld(4, 2); v1a = wld(4, 3); v0b = wld(5, 2); v1b = wld(5, 3);
-          tmem_wait_ld();
-          tmem_ld_16x256b_x8(ta_hi + 128, rb);
-          pass_c_piece<2>(ra, acc, w0a, w1a, w0b, w1b);
-          tmem_wait_ld();
-          if (n_chunks > 3) tmem_ld_16x256b_x8(ta + 192, ra);
-          pass_c_piece<2>(rb, acc, v0a, v1a, v0b, v1b);
-          if (n_chunks > 3) {
-            w0a = wld(6, 0); w1a = wld(6, 1); w0b = wld(7, 0); w1b = wld(7, 1);
-            v0a = wld(6, 2); v1a = wld(6, 3); v0b = wld(7, 2); v1b = wld(7, 3);
-            tmem_wait_ld();
-            tmem_ld_16x256b_x8(ta_hi + 192, rb);
-            pass_c_piece<3>(ra, acc, w0a, w1a, w0b, w1b);
-            tmem_wait_ld();
-            pass_c_piece<3>(rb, acc, v0a, v1a, v0b, v1b);
-          }
-        }
+        KARA_C_STEP(4) KARA_C_STEP(5) KARA_C_STEP(6) KARA_C_STEP(7)
+#undef KARA_C_STEP
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 1));
@@ -558,19 +546,31 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
   } else {
     // ================================ B warps: pass B ================================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(kRegsB));
-    // warp (q, cq) owns rows [32 q, 32 q + 32) and, in EACH MMA half, the 32-column piece cq: all 16 warps sweep
-    // half 0, then half 1, so the refill of a half has a whole half-sweep of slack and four warps per scheduler
-    // feed the MUFU pipe at any time
+    // Every thread owns, in EACH MMA half, one piece: 32 consecutive columns [32 pcq, + 32) of the half, of one S row.
+    // All 16 warps sweep half 0, then half 1, so the refill of a half has a whole half-sweep of slack and four warps per
+    // scheduler feed the MUFU pipe at any time.
     const int q = warp & 3, cq = warp >> 2;
-    const float cs = kLog2e * rsqrtf((float)D);
+#if KARA_B_SHAPE == 0
+    // 32x32b: warp (q, cq) holds rows [32 q, + 32) x piece column cq; thread = TMEM lane
+    const int pcq = cq, colw0 = cq * 32, colw_n = 32;
+    const int row = q * 32 + lane;
     const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 32;
+#else
+    // 16x32bx2: warp (q, cq) holds rows [32 q + 16 (cq & 1), + 16) x the 64 columns [64 (cq >> 1), + 64): thread t has row
+    // 32 q + 16 (cq & 1) + (t & 15), piece column 2 (cq >> 1) + (t >> 4)
+    const int pcq = 2 * (cq >> 1) + (lane >> 4), colw0 = (cq >> 1) * 64, colw_n = 64;
+    const int row = q * 32 + 16 * (cq & 1) + (lane & 15);
+    const uint32_t tq = tmem_base + ((uint32_t)(q * 32 + 16 * (cq & 1)) << 16) + (cq >> 1) * 64;
+#endif
+    const float cs = kLog2e * rsqrtf((float)D);
     int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
       const Seg it = decode_seg(c, g, g_end, rank, cluster_id, n_clusters, T, tpu);
       g += it.t1 - it.t0;
       if (!it.ok) continue;
       const int c_lo = it.c_lo, c_hi = it.c_hi;
-      const bool act0 = cq * 32 < it.n_cols, act1 = kHalf + cq * 32 < it.n_cols;   // the MMA writes this piece of half 0 / 1
+      // the MMA writes (some of) this warp's 64 columns of half 0 / 1 (a piece beyond them is masked as a whole)
+      const bool act0 = colw0 < it.n_cols, act1 = kHalf + colw0 < it.n_cols;
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
         const uint32_t ta = tq + b * kKeysPerCta;
@@ -581,7 +581,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 0);
         mbar_wait(tfull + 8 * (b * 2 + 0), par);
         tc_fence_after();
-        tmem_ld_32x32b_x32(ta, ra);                        // (an inactive piece is loaded too and ignored)
+        KARA_B_LD(ta, ra);                      // (an inactive piece is loaded too and ignored)
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 1);
         // the TMEM load of piece 1 runs under the exponentials of piece 0 (in the B-bound steady state its S half
         // has landed long before; a starved B warp loses at most the time between the two MMA halves here)
@@ -589,28 +589,28 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         mbar_wait(tfull + 8 * (b * 2 + 1), par);
         tc_fence_after();
         tmem_wait_ld();
-        tmem_ld_32x32b_x32(ta + kHalf, rb);
+        KARA_B_LD(ta + kHalf, rb);
 #else
         tmem_wait_ld();
 #endif
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 2);
         // ---- pass B: e = 2^(s c - z) in place; (z, l) of (row, piece); the thread owns row 32 q + lane ----
         if (act0) {
-          pass_b_piece(ra, z0, l0, cs, cq * 32, c_lo, c_hi);
-          tmem_st_32x32b_x32(ta, ra);
+          pass_b_piece(ra, z0, l0, cs, colw0, colw_n, pcq * 32, c_lo, c_hi);
+          KARA_B_ST(ta, ra);
         }
 #if !KARA_B_PREFETCH
         mbar_wait(tfull + 8 * (b * 2 + 1), par);
         tc_fence_after();
-        tmem_ld_32x32b_x32(ta + kHalf, rb);
+        KARA_B_LD(ta + kHalf, rb);
 #endif
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 3);
         tmem_wait_ld();
         if (act1) {
-          pass_b_piece(rb, z1, l1, cs, kHalf + cq * 32, c_lo, c_hi);
-          tmem_st_32x32b_x32(ta + kHalf, rb);
+          pass_b_piece(rb, z1, l1, cs, kHalf + colw0, colw_n, kHalf + pcq * 32, c_lo, c_hi);
+          KARA_B_ST(ta + kHalf, rb);
         }
-        rstat[(b * 4 + cq) * 128 + q * 32 + lane] = make_uint4((uint32_t)z0, __float_as_uint(l0), (uint32_t)z1, __float_as_uint(l1));
+        rstat[(b * 4 + pcq) * 128 + row] = make_uint4((uint32_t)z0, __float_as_uint(l0), (uint32_t)z1, __float_as_uint(l1));
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 4);
         tmem_wait_st();
         tc_fence_before();

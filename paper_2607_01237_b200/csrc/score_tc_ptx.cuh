@@ -219,6 +219,24 @@ __device__ __forceinline__ void tmem_st_32x32b_x32(uint32_t taddr, const uint32_
       "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
       :: KARA_TMEM_IN32(r), "r"(taddr) : "memory");
 }
+// 16 lanes x (32 + 32) columns: thread t < 16 gets lane t, columns [c, c+32); thread t >= 16 gets lane t-16, columns
+// [c+32, c+64) — one S row piece of 32 consecutive columns per thread.  (The 32x32b shape, one lane per thread, would
+// give a thread its row directly, but measured on B200 it reads TMEM at 57 B/clk per SM however many warps issue it;
+// the 16-lane shapes reach 200+ B/clk: _work microbenchmark.)
+__device__ __forceinline__ void tmem_ld_16x32bx2_x32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.16x32bx2.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32], 32;"
+      : KARA_TMEM_REGS32(r) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st_16x32bx2_x32(uint32_t taddr, const uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.16x32bx2.x32.b32 [%32], 32, "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
+      :: KARA_TMEM_IN32(r), "r"(taddr) : "memory");
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
