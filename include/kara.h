@@ -131,6 +131,23 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
                          unsigned flags, void* workspace /*dev*/, size_t workspace_bytes,
                          void* stream);
 
+/* Prefill / multi-window batch (App. C.2: "partition the prompt into multiple windows of length |W| and
+ * perform window-wise compression ... in parallel"; L346).  Reading G17: the n_windows windows of a sequence
+ * are the disjoint ranges [h + w W, h + (w+1) W), h = win_start[s] (NULL => seq_len - n_windows*W); each is scored with its
+ * own W queries against its own n keys and selected on its own (a1-a3 unchanged); a4 lays the retained rows and the buffer
+ * of window w down behind those of window w-1 and the t = seq_len - h - n_windows*W tail rows behind the last window:
+ *     new[h + w (keep+U) + c]        = old[h + w W + F_w[c]]    c < keep
+ *     new[h + w (keep+U) + keep + c] = old[h + w W + n + c]     c < U
+ *     new[h + n_windows (keep+U) + c] = old[h + n_windows W + c]   c < t
+ * a5: seq_len <- h + n_windows (keep+U) + t.  window_q is [layers x n_seqs x n_windows*W x n_q_heads x head_dim]; the
+ * workspace must hold kara_workspace_bytes(..., n_seqs * n_windows, ...) bytes; after such a call the `seq` argument of
+ * kara_gather_debug(SCORES / IDX_*) is sequence * n_windows + window.  n_windows = 1 is kara_compress_window. */
+int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_seqs,
+                          int32_t* block_table /*dev*/, int max_blocks, int32_t* seq_lens /*dev*/,
+                          const int32_t* win_start /*dev or NULL*/, int n_windows, const void* window_q /*dev*/,
+                          int n_q_heads, int W, int U, double ratio, int alpha, int gamma,
+                          unsigned flags, void* workspace /*dev*/, size_t workspace_bytes, void* stream);
+
 /* Same step with HOST buffers for everything but the resident pools: copies window_q,
  * block_table, seq_lens, win_start host->device into library-owned staging buffers, runs
  * kara_compress_window on `stream`, copies block_table and seq_lens back and reports the new

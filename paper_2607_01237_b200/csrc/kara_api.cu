@@ -197,7 +197,16 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
                          int max_blocks, int32_t* seq_lens, const int32_t* win_start, const void* window_q,
                          int n_q_heads, int W, int U, double ratio, int alpha, int gamma, unsigned flags,
                          void* workspace, size_t workspace_bytes, void* stream) {
+  return kara_compress_windows(c, layer_begin, layer_end, n_seqs, block_table, max_blocks, seq_lens, win_start, 1,
+                               window_q, n_q_heads, W, U, ratio, alpha, gamma, flags, workspace, workspace_bytes, stream);
+}
+
+int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_seqs, int32_t* block_table,
+                          int max_blocks, int32_t* seq_lens, const int32_t* win_start, int n_windows,
+                          const void* window_q, int n_q_heads, int W, int U, double ratio, int alpha, int gamma,
+                          unsigned flags, void* workspace, size_t workspace_bytes, void* stream) {
   int keep = 0;
+  if (n_windows < 1) return fail(KARA_EINVAL, "n_windows=%d", n_windows);
   int rc = check_geometry(c, layer_begin, layer_end, n_seqs, n_q_heads, W, U, ratio, alpha, gamma, &keep);
   if (rc != KARA_OK) return rc;
   if (!c->attached) return fail(KARA_EINVAL, "kara_attach_pool has not been called");
@@ -209,7 +218,7 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
 
   const int nL = layer_end - layer_begin;
   const int n = W - U;
-  const int units = nL * n_seqs * c->g.n_kv_heads;
+  const int units = nL * n_seqs * n_windows * c->g.n_kv_heads;
   const WsLayout w = ws_layout(units, n, keep - alpha, keep, (W + 127) / 128 * (n_q_heads / c->g.n_kv_heads));
   if (workspace_bytes < w.total)
     return fail(KARA_ENOMEM, "workspace %zu bytes < %zu needed", workspace_bytes, w.total);
@@ -221,6 +230,7 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   k.layer_begin = layer_begin;
   k.n_layers = nL;
   k.n_seqs = n_seqs;
+  k.n_windows = n_windows;
   k.max_blocks = max_blocks;
   k.n_q_heads = n_q_heads;
   k.G = n_q_heads / c->g.n_kv_heads;
@@ -280,6 +290,10 @@ int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_se
   // ---- a2-a4 select + Token2Chunk + compaction ---------------------------------------------------
   KARA_CUDA(launch_select_compact(k, st));
   ++launches;
+  if (n_windows > 1) {      // prefill: the rows of all windows of a (layer, sequence, head) are moved by one CTA, in window order
+    KARA_CUDA(launch_compact_windows(k, st));
+    ++launches;
+  }
 
   // ---- a5 metadata ---------------------------------------------------------------------------------
   if (flags & KARA_COMMIT) {
@@ -398,9 +412,10 @@ int kara_gather_debug(kara_cache* c, int what, int layer, int seq, int kv_head, 
         return fail(KARA_EINVAL, "no previous kara_compress_window call with KARA_KEEP_DEBUG");
       const Call& k = c->last;
       const int li = layer - k.layer_begin;
-      if (li < 0 || li >= k.n_layers || seq < 0 || seq >= k.n_seqs || kv_head < 0 || kv_head >= k.g.n_kv_heads)
+      // after a multi-window call `seq` is sequence * n_windows + window (include/kara.h)
+      if (li < 0 || li >= k.n_layers || seq < 0 || seq >= k.n_seqs * k.n_windows || kv_head < 0 || kv_head >= k.g.n_kv_heads)
         return fail(KARA_EINVAL, "unit (layer=%d, seq=%d, head=%d) not in the last call", layer, seq, kv_head);
-      const int64_t unit = ((int64_t)li * k.n_seqs + seq) * k.g.n_kv_heads + kv_head;
+      const int64_t unit = ((int64_t)li * k.n_seqs * k.n_windows + seq) * k.g.n_kv_heads + kv_head;
       if (what == KARA_DBG_SCORES) return copy_out(k.scores + unit * k.n_pad, k.n, 4);
       if (what == KARA_DBG_IDX_TOPK) return copy_out(k.idx_topk + unit * k.k_pad, k.k, 4);
       return copy_out(k.idx_final + unit * k.keep_pad, k.keep, 4);

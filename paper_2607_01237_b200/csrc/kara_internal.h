@@ -23,6 +23,7 @@ struct Call {
   const __nv_bfloat16* k_pool;
   const __nv_bfloat16* v_pool;  // written by the compaction kernel through a non-const alias
   int layer_begin, n_layers, n_seqs, max_blocks;
+  int n_windows;    // NW >= 1 disjoint windows of W tokens per sequence (prefill, App. C.2; 1 = the decoding-time step)
   int n_q_heads, G, W, U, n, keep, k, P, alpha, gamma;
   int q_row_begin;  // first window token used as a query (0, or W-U with KARA_SCORE_QBUF_ONLY)
   int32_t* block_table;
@@ -79,19 +80,24 @@ inline int strips_bound(int units, int tpu) {
   return (int)(kScoreStrips * ranges);
 }
 
-// unit index -> (layer-in-call, sequence, kv head)
-__host__ __device__ inline void unit_decode(int unit, int n_seqs, int n_kv_heads, int& li, int& s, int& hk) {
+// unit index -> (layer-in-call, sequence, window, kv head); units are ordered ((layer, sequence), window, kv head)
+__host__ __device__ inline void unit_decode(int unit, int n_seqs, int n_windows, int n_kv_heads, int& li, int& s, int& w,
+                                            int& hk) {
   hk = unit % n_kv_heads;
-  s = (unit / n_kv_heads) % n_seqs;
-  li = unit / (n_kv_heads * n_seqs);
+  unit /= n_kv_heads;
+  w = unit % n_windows;
+  unit /= n_windows;
+  s = unit % n_seqs;
+  li = unit / n_seqs;
 }
+__host__ __device__ inline int unit_count(const Call& c) { return c.n_layers * c.n_seqs * c.n_windows * c.g.n_kv_heads; }
 
-// Window geometry of sequence s, validated on the device.  Returns false (and sets status bits)
-// if the unit must be skipped.
+// Window geometry of sequence s, validated on the device: h = first token of its FIRST window, t = tail tokens behind its
+// last window (window w covers [h + w W, h + (w+1) W)).  Returns false (and sets status bits) if the sequence must be skipped.
 __device__ inline bool window_of(const Call& c, int s, int& h, int& t, int& len) {
   len = c.seq_lens[s];
-  h = c.win_start ? c.win_start[s] : len - c.W;
-  t = len - h - c.W;
+  h = c.win_start ? c.win_start[s] : len - c.n_windows * c.W;
+  t = len - h - c.n_windows * c.W;
   int bad = 0;
   if (h < 0 || t < 0) bad |= KARA_ST_SHORT_SEQ;
   if (((len + c.g.bs - 1) >> c.g.bs_log2) > c.max_blocks) bad |= KARA_ST_TABLE_OVERFLOW;
@@ -128,6 +134,7 @@ __device__ inline long long row_offset(const Call& c, int layer, int s, int hk, 
 // kernel launchers (each returns the cudaError_t of its launch)
 cudaError_t launch_score_simt(const Call& c, cudaStream_t st);
 cudaError_t launch_select_compact(const Call& c, cudaStream_t st);
+cudaError_t launch_compact_windows(const Call& c, cudaStream_t st);   // a4 of a multi-window call (n_windows > 1)
 cudaError_t launch_metadata(const Call& c, cudaStream_t st);
 cudaError_t launch_gather_rows(const Geom& g, const __nv_bfloat16* pool, int layer, int kv_head,
                                const int32_t* bt_row, int length, __nv_bfloat16* out, int32_t* status,

@@ -2,7 +2,7 @@
 // App. C.4), and the logical-row gather behind kara_gather_debug.
 //
 // One CTA walks the sequences in batch order, 256 at a time: per sequence
-//   new_len = h + keep + U + t,  new_nb = ceil(new_len / bs),  old_nb = ceil(len / bs)
+//   new_len = h + NW (keep + U) + t,  new_nb = ceil(new_len / bs),  old_nb = ceil(len / bs)     (NW = windows per sequence)
 // the freed counts are exclusive-scanned so that block_table[s][new_nb:old_nb] lands on the free
 // list in sequence order, table order (reading G16: a deterministic scan, not atomics, so the
 // list is bit-comparable with the oracle's).
@@ -27,8 +27,8 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
     bool ok = false;
     if (s < c.n_seqs) {
       const int len = c.seq_lens[s];
-      const int h = c.win_start ? c.win_start[s] : len - c.W;
-      const int t = len - h - c.W;
+      const int h = c.win_start ? c.win_start[s] : len - c.n_windows * c.W;
+      const int t = len - h - c.n_windows * c.W;
       old_nb = (len + c.g.bs - 1) >> c.g.bs_log2;
       ok = (h >= 0 && t >= 0 && old_nb <= c.max_blocks);
       if (ok) {
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
         if (!ok) atomicOr(c.status, KARA_ST_BAD_BLOCK);
       }
       if (ok) {
-        new_len = h + c.keep + c.U + t;
+        new_len = h + c.n_windows * (c.keep + c.U) + t;   // every window leaves keep + U rows behind
         new_nb = (new_len + c.g.bs - 1) >> c.g.bs_log2;
         freed = old_nb - new_nb;
       }

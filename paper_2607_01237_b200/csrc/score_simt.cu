@@ -36,14 +36,15 @@ __global__ void __launch_bounds__(kThreads) score_simt_kernel(const Call c) {
   long long* s_koff = reinterpret_cast<long long*>(s_q + kWarps * d);  // [n_pad] key row offsets
 
   const int unit = blockIdx.x, part = blockIdx.y;
-  int li, s, hk;
-  unit_decode(unit, c.n_seqs, c.g.n_kv_heads, li, s, hk);
+  int li, s, w, hk;
+  unit_decode(unit, c.n_seqs, c.n_windows, c.g.n_kv_heads, li, s, w, hk);
   const int layer = c.layer_begin + li;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   float* out = c.partial + ((long long)unit * c.parts + part) * n_pad;
 
   int h, t, len;
   const bool ok = window_of(c, s, h, t, len);
+  h += w * c.W;                                            // this unit's window
   for (int j = threadIdx.x; j < n; j += kThreads) s_koff[j] = ok ? row_offset(c, layer, s, hk, h + j) : -1;
   for (int j = threadIdx.x; j < kWarps * n_pad; j += kThreads) s_acc[j] = 0.f;
   __syncthreads();
@@ -66,7 +67,7 @@ __global__ void __launch_bounds__(kThreads) score_simt_kernel(const Call c) {
   for (int r = r0 + warp; r < r1; r += kWarps) {
     const int i = c.q_row_begin + r / c.G, g = r % c.G;
     const __nv_bfloat16* q = c.window_q +
-        ((((long long)li * c.n_seqs + s) * c.W + i) * c.n_q_heads + (hk * c.G + g)) * (long long)d;
+        (((((long long)li * c.n_seqs + s) * c.n_windows + w) * c.W + i) * c.n_q_heads + (hk * c.G + g)) * (long long)d;
     for (int x = lane; x < d; x += 32) my_q[x] = __bfloat162float(q[x]);
     __syncwarp();
     float m = -INFINITY;
@@ -112,7 +113,7 @@ __global__ void __launch_bounds__(kThreads) score_simt_kernel(const Call c) {
 }  // namespace
 
 cudaError_t launch_score_simt(const Call& c, cudaStream_t st) {
-  const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;
+  const int units = unit_count(c);
   const size_t smem = sizeof(float) * (size_t)(2 * kWarps * c.n_pad + kWarps * c.g.d) +
                       sizeof(long long) * (size_t)c.n_pad;
   cudaError_t e = cudaFuncSetAttribute(score_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -104,7 +104,7 @@ struct Smem {
 
 // One segment: the tiles [t0, t1) of `unit` that fall into this cluster's range.
 struct Seg {
-  int unit, part, li, s, hk, layer;
+  int unit, part, li, s, w, hk, layer;
   int h, fb, off;          // window start, first key block (table index), h - fb*bs
   int c_lo, c_hi;          // this CTA's valid key columns [c_lo, c_hi) within its 256
   int n_cols;              // columns the MMAs of this CTA produce: valid columns rounded up to 16 (>= 16)
@@ -120,13 +120,13 @@ __device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long 
   const long long left = g_end - g;
   it.t1 = (int)(left < (long long)(tpu - it.t0) ? it.t0 + left : tpu);
   it.part = cluster_id - tile_owner((long long)it.unit * tpu, n_clusters, T);
-  unit_decode(it.unit, c.n_seqs, c.g.n_kv_heads, it.li, it.s, it.hk);
+  unit_decode(it.unit, c.n_seqs, c.n_windows, c.g.n_kv_heads, it.li, it.s, it.w, it.hk);
   it.layer = c.layer_begin + it.li;
   const int len = c.seq_lens[it.s];
-  it.h = c.win_start ? c.win_start[it.s] : len - c.W;
-  const int t = len - it.h - c.W;
-  it.ok = (it.h >= 0 && t >= 0 && ((len + c.g.bs - 1) >> c.g.bs_log2) <= c.max_blocks);
-  if (!it.ok) it.h = 0;
+  const int h0 = c.win_start ? c.win_start[it.s] : len - c.n_windows * c.W;   // first window of the sequence
+  const int t = len - h0 - c.n_windows * c.W;
+  it.ok = (h0 >= 0 && t >= 0 && ((len + c.g.bs - 1) >> c.g.bs_log2) <= c.max_blocks);
+  it.h = it.ok ? h0 + it.w * c.W : 0;
   it.fb = it.h >> c.g.bs_log2;
   it.off = it.h - (it.fb << c.g.bs_log2);
   // panel row pr = rank*256 + col  <->  window-relative key j = pr - off ; valid iff 0 <= j < n
@@ -320,7 +320,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           mbar_wait_backoff(qempty + 8 * stage, (use & 1) ^ 1);
           mbar_expect_tx(qfull + 8 * stage, SM::kQStageBytes);
           const int gq = tile / tok_tiles, tt = tile % tok_tiles;
-          const int tok = (cur.li * c.n_seqs + cur.s) * c.W + c.q_row_begin + tt * kTileM;
+          const int tok = ((cur.li * c.n_seqs + cur.s) * c.n_windows + cur.w) * c.W + c.q_row_begin + tt * kTileM;
 #pragma unroll
           for (int p = 0; p < SM::kPanels; ++p)
             tma_load_3d(sQ + stage * SM::kQStageBytes + p * (kTileM * 128), &q_map, qfull + 8 * stage,
@@ -667,7 +667,7 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
     return tc_fail(KARA_ECUDA, "cudaFuncSetAttribute(max dynamic smem) failed");
   const int tok_tiles = (c.W - c.q_row_begin + kTileM - 1) / kTileM;
   const int tpu = tok_tiles * c.G;
-  const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;
+  const int units = unit_count(c);
   const long long T = (long long)units * tpu;
   if (T >= (1ll << 31)) return tc_fail(KARA_EUNSUPPORTED, "more than 2^31 query tiles in one call");
 
@@ -749,14 +749,14 @@ bool score_tc_supported(const ScoreTcState& s, const Call& c) {
   if (c.g.d != 64 && c.g.d != 128) return false;
   if (c.g.bs > kKeysPerCta) return false;
   if (cluster_size_for(c) == 0) return false;
-  const unsigned long long toks = (unsigned long long)c.n_layers * c.n_seqs * c.W;
+  const unsigned long long toks = (unsigned long long)c.n_layers * c.n_seqs * c.n_windows * c.W;
   if (toks >= (1ull << 31)) return false;
   return true;
 }
 
 int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) {
   // window_q tensor map: [d][n_q_heads][layers*seqs*W tokens], box 64 x 1 x 128, 128B swizzle
-  const long long key[6] = {(long long)(uintptr_t)c.window_q, c.g.d, c.n_q_heads, (long long)c.n_layers * c.n_seqs * c.W, 0, 0};
+  const long long key[6] = {(long long)(uintptr_t)c.window_q, c.g.d, c.n_q_heads, (long long)c.n_layers * c.n_seqs * c.n_windows * c.W, 0, 0};
   if (s->q_ptr != c.window_q || memcmp(key, s->q_key, sizeof key) != 0) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return tc_fail(KARA_ECUDA, "cuTensorMapEncodeTiled entry point not found");

@@ -12,6 +12,10 @@
 // index order with a ballot-free segmented count + block scan.  All decisions are integer
 // compares on fp32 bit patterns, so the result is a pure function of the scores.
 //
+// Prefill (n_windows > 1, App. C.2): the select kernel runs per (layer, sequence, window, head) unit and only
+// writes F; compact_windows_kernel then moves the rows of ALL windows of a (layer, sequence, head) with one CTA, window by
+// window, each window's retained rows + buffer laid down behind those of the window before it.
+//
 // In-place compaction is hazard-free with one CTA per unit: destination c <= source F[c] and both
 // are increasing, so loading rows [c0,c1) into registers, barrier, then writing them never
 // overwrites a row a later chunk still has to read.
@@ -149,16 +153,59 @@ __device__ __forceinline__ void st_na16(void* p, const uint4& v) {
                :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// a4: rows src_of(r) -> h + r for r in [0, moved), K and V together, in place, staged through REGISTERS.
+// A chunk of rows_per_pass rows of K and of V is loaded completely (every thread holds its 16-byte vectors in
+// registers: all loads of the chunk are in flight together), the block synchronises, then the chunk is written.
+// src_of is increasing with src_of(r) >= h + r, so a chunk's writes never touch a row a later chunk still has
+// to read.  Block-wide; s_off = [2][stage_rows] row offsets in shared memory.
+template <typename SrcOf>
+__device__ __forceinline__ void compact_rows_inplace(const Call& c, int layer, int s, int hk, int h, int moved, SrcOf src_of,
+                                                     long long* s_off, int stage_rows) {
+  const int tid = threadIdx.x;
+  const int vpr = c.g.d / 8;                                   // 16-byte vectors per row
+  constexpr int kVecPerThread = 8;                             // per tensor
+  const int rows_per_pass = kThreads * kVecPerThread / vpr;    // 128 rows at d = 128, 256 at d = 64
+  __nv_bfloat16* kp = const_cast<__nv_bfloat16*>(c.k_pool);
+  __nv_bfloat16* vp = const_cast<__nv_bfloat16*>(c.v_pool);
+  for (int c0 = 0; c0 < moved; c0 += rows_per_pass) {
+    const int rows = min(rows_per_pass, moved - c0);
+    // the block-table walk once per row (the same for K and V), not once per 16-byte vector
+    for (int r = tid; r < rows; r += kThreads) {
+      const int row = c0 + r;
+      s_off[r] = row_offset(c, layer, s, hk, src_of(row));
+      s_off[stage_rows + r] = row_offset(c, layer, s, hk, h + row);
+    }
+    __syncthreads();
+    uint4 kv[kVecPerThread], vv[kVecPerThread];
+#pragma unroll
+    for (int u = 0; u < kVecPerThread; ++u) {
+      const int x = tid + u * kThreads;
+      const int r = x / vpr, v = x % vpr;
+      const long long off = r < rows ? s_off[r] : -1;
+      kv[u] = off >= 0 ? __ldcg(reinterpret_cast<const uint4*>(kp + off + v * 8)) : make_uint4(0, 0, 0, 0);
+      vv[u] = off >= 0 ? __ldcg(reinterpret_cast<const uint4*>(vp + off + v * 8)) : make_uint4(0, 0, 0, 0);
+    }
+    __syncthreads();                                           // every read of the chunk has completed
+#pragma unroll
+    for (int u = 0; u < kVecPerThread; ++u) {
+      const int x = tid + u * kThreads;
+      const int r = x / vpr, v = x % vpr;
+      const long long off = r < rows ? s_off[stage_rows + r] : -1;
+      if (off >= 0) { st_na16(kp + off + v * 8, kv[u]); st_na16(vp + off + v * 8, vv[u]); }
+    }
+    __syncthreads();
+  }
+}
+
 __global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call c, int stage_rows, int off_bytes) {
   // programmatic dependent launch: this grid may be scheduled while the score kernel drains; nothing the
   // score kernel writes is read before the wait, and the metadata kernel behind may be scheduled early too
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int n = c.n, n_pad = c.n_pad, k = c.k, keep = c.keep, d = c.g.d;
+  const int n = c.n, n_pad = c.n_pad, k = c.k, keep = c.keep;
   // carve
   unsigned char* s_fill = smem_raw;                                            // [n_pad] fill flags
-  const int vpr = d / 8;                                                       // 16-byte vectors per row
   float* s_A = reinterpret_cast<float*>(smem_raw + ((n_pad + 15) / 16) * 16);  // [n_pad]
   unsigned* s_key = reinterpret_cast<unsigned*>(s_A + n_pad);                  // [n_pad]
   int* s_I = reinterpret_cast<int*>(s_key + n_pad);                            // [k_pad]
@@ -171,11 +218,11 @@ __global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call 
   long long* s_off = reinterpret_cast<long long*>(smem_raw + off_bytes);       // [2][stage_rows] src / dst offsets
 
   const int unit = blockIdx.x, tid = threadIdx.x;
-  int li, s, hk;
-  unit_decode(unit, c.n_seqs, c.g.n_kv_heads, li, s, hk);
+  int li, s, w, hk;
+  unit_decode(unit, c.n_seqs, c.n_windows, c.g.n_kv_heads, li, s, w, hk);
   const int layer = c.layer_begin + li;
 
-  int h, t, len;
+  int h, t, len;                             // h = first window of the sequence, t = tail behind the last one
   if (!window_of(c, s, h, t, len)) return;   // uniform per CTA
   // every table entry of the window is validated BEFORE anything is written: a sequence with a block id
   // outside the pool is skipped as a whole (no compaction here, no metadata update in a5)
@@ -252,47 +299,41 @@ __global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call 
     __syncthreads();
   }
   block_compact(s_sel, n, s_F, sc);   // F: ascending (reading G10), |F| = keep
-  if (c.keep_debug) for (int x = tid; x < keep; x += kThreads) c.idx_final[(long long)unit * c.keep_pad + x] = s_F[x];
+  // F goes to the workspace for kara_gather_debug and, in a multi-window call, for compact_windows_kernel
+  if (c.keep_debug || c.n_windows > 1)
+    for (int x = tid; x < keep; x += kThreads) c.idx_final[(long long)unit * c.keep_pad + x] = s_F[x];
+  if (c.n_windows > 1) return;               // a4 of a multi-window call: compact_windows_kernel
 
-  // ---- a4: compaction of K and V (Eq. 9), staged through REGISTERS -----------------------------
-  // A chunk of kRowsPerPass rows of K and of V is loaded completely (every thread holds its 16-byte
-  // vectors in registers: all loads of the chunk are in flight together), the block synchronises, then
-  // the chunk is written.  Destination row c <= source row F[c], both increasing, so a chunk's writes
-  // never touch a row a later chunk still has to read.
-  const int moved = keep + c.U + t;
-  constexpr int kVecPerThread = 8;                             // per tensor
-  const int rows_per_pass = kThreads * kVecPerThread / vpr;    // 128 rows at d = 128, 256 at d = 64
-  __nv_bfloat16* kp = const_cast<__nv_bfloat16*>(c.k_pool);
-  __nv_bfloat16* vp = const_cast<__nv_bfloat16*>(c.v_pool);
-  for (int c0 = 0; c0 < moved; c0 += rows_per_pass) {
-    const int rows = min(rows_per_pass, moved - c0);
-    // the block-table walk once per row (the same for K and V), not once per 16-byte vector
-    for (int r = tid; r < rows; r += kThreads) {
-      const int row = c0 + r;
-      const int src = row < keep ? h + s_F[row] : h + n + (row - keep);
-      s_off[r] = row_offset(c, layer, s, hk, src);
-      s_off[stage_rows + r] = row_offset(c, layer, s, hk, h + row);
-    }
-    __syncthreads();
-    uint4 kv[kVecPerThread], vv[kVecPerThread];
-#pragma unroll
-    for (int u = 0; u < kVecPerThread; ++u) {
-      const int x = tid + u * kThreads;
-      const int r = x / vpr, v = x % vpr;
-      const long long off = r < rows ? s_off[r] : -1;
-      kv[u] = off >= 0 ? __ldcg(reinterpret_cast<const uint4*>(kp + off + v * 8)) : make_uint4(0, 0, 0, 0);
-      vv[u] = off >= 0 ? __ldcg(reinterpret_cast<const uint4*>(vp + off + v * 8)) : make_uint4(0, 0, 0, 0);
-    }
-    __syncthreads();                                           // every read of the chunk has completed
-#pragma unroll
-    for (int u = 0; u < kVecPerThread; ++u) {
-      const int x = tid + u * kThreads;
-      const int r = x / vpr, v = x % vpr;
-      const long long off = r < rows ? s_off[stage_rows + r] : -1;
-      if (off >= 0) { st_na16(kp + off + v * 8, kv[u]); st_na16(vp + off + v * 8, vv[u]); }
-    }
-    __syncthreads();
-  }
+  // ---- a4: compaction of K and V (Eq. 9): rows h + F[c] -> h + c, buffer + tail rows behind them ----
+  const int* F = s_F;
+  compact_rows_inplace(c, layer, s, hk, h, keep + c.U + t,
+                       [=](int row) { return row < keep ? h + F[row] : h + n + (row - keep); }, s_off, stage_rows);
+}
+
+// a4 of a multi-window call (App. C.2, reading G17): one CTA per (layer, sequence, KV head) moves, in window order,
+//   new[h + w (keep+U) + c]        = old[h + w W + F_w[c]]       c < keep
+//   new[h + w (keep+U) + keep + c] = old[h + w W + n + c]        c < U
+//   new[h + NW (keep+U) + c]       = old[h + NW W + c]           c < t
+// F_w is read from the workspace (written by select_compact_kernel of the same call).
+__global__ void __launch_bounds__(kThreads, 3) compact_windows_kernel(const Call c, int stage_rows) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  long long* s_off = reinterpret_cast<long long*>(smem_raw);
+  const int NW = c.n_windows, Hkv = c.g.n_kv_heads;
+  const int hk = blockIdx.x % Hkv, s = (blockIdx.x / Hkv) % c.n_seqs, li = blockIdx.x / (Hkv * c.n_seqs);
+  int h, t, len;
+  if (!window_of(c, s, h, t, len)) return;
+  if (!window_blocks_ok(c, s, h, len)) return;
+  const int keep = c.keep, per = c.keep + c.U, n = c.n, W = c.W;
+  const int32_t* F = c.idx_final + ((((long long)li * c.n_seqs + s) * NW) * Hkv + hk) * c.keep_pad;   // window 0
+  const long long f_stride = (long long)Hkv * c.keep_pad;                                            // to the next window
+  compact_rows_inplace(c, c.layer_begin + li, s, hk, h, NW * per + t,
+                       [=](int row) {
+                         if (row >= NW * per) return h + NW * W + (row - NW * per);       // tail
+                         const int w = row / per, x = row - w * per;
+                         return x < keep ? h + w * W + F[w * f_stride + x] : h + w * W + n + (x - keep);
+                       }, s_off, stage_rows);
 }
 
 size_t smem_bytes(const Call& c) {
@@ -307,7 +348,7 @@ size_t smem_bytes(const Call& c) {
 }  // namespace
 
 cudaError_t launch_select_compact(const Call& c, cudaStream_t st) {
-  const int units = c.n_layers * c.n_seqs * c.g.n_kv_heads;
+  const int units = unit_count(c);
   // offset table: one pass of the compaction moves 256 x 8 vectors per tensor = at most 256 rows (d = 64)
   const int stage_rows = 256;
   const size_t off_bytes = smem_bytes(c);
@@ -323,6 +364,19 @@ cudaError_t launch_select_compact(const Call& c, cudaStream_t st) {
   cfg.gridDim = dim3(units); cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = smem; cfg.stream = st;
   return cudaLaunchKernelEx(&cfg, select_compact_kernel, c, stage_rows, (int)off_bytes);
+}
+
+cudaError_t launch_compact_windows(const Call& c, cudaStream_t st) {
+  const int stage_rows = 256;
+  const size_t smem = 2 * sizeof(long long) * (size_t)stage_rows;
+  cudaLaunchConfig_t cfg{};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cfg.gridDim = dim3(c.n_layers * c.n_seqs * c.g.n_kv_heads); cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  return cudaLaunchKernelEx(&cfg, compact_windows_kernel, c, stage_rows);
 }
 
 }  // namespace kara

@@ -35,6 +35,8 @@ SYMBOLS = {
     "kara_workspace_bytes": (_sz, [_vp, _i, _i, _i, _i, _i, _d, _i]),
     "kara_compress_window": (_i, [_vp, _i, _i, _i, _vp, _i, _vp, _vp, _vp, _i, _i, _i, _d, _i, _i, _u,
                                   _vp, _sz, _vp]),
+    "kara_compress_windows": (_i, [_vp, _i, _i, _i, _vp, _i, _vp, _vp, _i, _vp, _i, _i, _i, _d, _i, _i, _u,
+                                   _vp, _sz, _vp]),
     "kara_compress_window_host": (_i, [_vp, _i, _i, _i, _vp, _i, _vp, _vp, _vp, _i, _i, _i, _d, _i, _i,
                                        _u, _vp, _vp]),
     "kara_gather_debug": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i, _vp, _i64, C.POINTER(_i64)]),
@@ -148,6 +150,25 @@ class KaraCache:
         _check(lib().kara_compress_window(self._h, layer_begin, layer_end, n_seqs, _ptr(block_table), max_blocks,
                                           _ptr(seq_lens), _ptr(win_start), _ptr(window_q), Hq, W, U, float(ratio),
                                           alpha, gamma, flags, _ptr(workspace), workspace.numel(), st))
+
+    # -- kara_compress_windows (prefill: n_windows disjoint windows per sequence) ---------------------------
+    def compress_windows(self, layer_begin: int, layer_end: int, block_table: torch.Tensor, seq_lens: torch.Tensor,
+                         win_start: torch.Tensor | None, n_windows: int, window_q: torch.Tensor, W: int, U: int,
+                         ratio: float, alpha: int, gamma: int, flags: int = KARA_COMMIT,
+                         workspace: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None) -> None:
+        n_seqs, max_blocks = block_table.shape
+        nL, S, Wq, Hq, d = window_q.shape
+        assert (nL, S, Wq, d) == (layer_end - layer_begin, n_seqs, n_windows * W, self.head_dim), "window_q shape"
+        assert window_q.is_cuda and window_q.is_contiguous() and window_q.dtype == torch.bfloat16
+        assert block_table.dtype == torch.int32 and block_table.is_contiguous() and block_table.is_cuda
+        assert seq_lens.dtype == torch.int32 and seq_lens.is_cuda
+        if workspace is None:
+            workspace = self._get_workspace(self.workspace_bytes(nL, n_seqs * n_windows, Hq, W, U, ratio, alpha),
+                                            window_q.device)
+        st = (stream or torch.cuda.current_stream(window_q.device)).cuda_stream
+        _check(lib().kara_compress_windows(self._h, layer_begin, layer_end, n_seqs, _ptr(block_table), max_blocks,
+                                           _ptr(seq_lens), _ptr(win_start), n_windows, _ptr(window_q), Hq, W, U,
+                                           float(ratio), alpha, gamma, flags, _ptr(workspace), workspace.numel(), st))
 
     # -- kara_compress_window_host -------------------------------------------------------------------
     def compress_window_host(self, layer_begin: int, layer_end: int, block_table: torch.Tensor,

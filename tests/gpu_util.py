@@ -32,25 +32,30 @@ def gpu_compress(wl, layer_begin=None, layer_end=None, flags=kara.KARA_COMMIT | 
     le = L if layer_end is None else layer_end
     cache = kara.KaraCache(sh.block_size, L, sh.n_kv_heads, sh.head_dim)
     cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
-    cache.compress_window(lb, le, D["bt"], D["sl"], D["ws"] if use_win_start else None,
-                          D["q"][lb:le].contiguous(), p["W"], p["U"], p["ratio"], p["alpha"], p["gamma"], flags)
+    NW = getattr(sh, "n_windows", 1)
+    if NW > 1:      # prefill: kara_compress_windows
+        cache.compress_windows(lb, le, D["bt"], D["sl"], D["ws"] if use_win_start else None, NW,
+                               D["q"][lb:le].contiguous(), p["W"], p["U"], p["ratio"], p["alpha"], p["gamma"], flags)
+    else:
+        cache.compress_window(lb, le, D["bt"], D["sl"], D["ws"] if use_win_start else None,
+                              D["q"][lb:le].contiguous(), p["W"], p["U"], p["ratio"], p["alpha"], p["gamma"], flags)
     torch.cuda.synchronize()
-    out = readback(cache, D, lb, le, sh.n_seqs, sh.n_kv_heads, flags)
+    out = readback(cache, D, lb, le, sh.n_seqs, sh.n_kv_heads, flags, n_windows=NW)
     return out, cache, D
 
 
-def readback(cache, D, lb, le, n_seqs, n_kv_heads, flags):
+def readback(cache, D, lb, le, n_seqs, n_kv_heads, flags, n_windows=1):
     out = dict(k=bits(D["k"]), v=bits(D["v"]), bt=D["bt"].cpu().numpy().copy(), sl=D["sl"].cpu().numpy().copy(),
                fl=D["fl"].cpu().numpy().copy(), fc=D["fc"].cpu().numpy().copy(), status=cache.status())
     if flags & kara.KARA_KEEP_DEBUG:
         sc, it, fi = [], [], []
         for l in range(lb, le):
-            for s in range(n_seqs):
+            for s in range(n_seqs * n_windows):      # after a multi-window call `seq` is sequence * n_windows + window
                 for hk in range(n_kv_heads):
                     sc.append(cache.gather_debug(kara.KARA_DBG_SCORES, l, s, hk))
                     it.append(cache.gather_debug(kara.KARA_DBG_IDX_TOPK, l, s, hk))
                     fi.append(cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, s, hk))
-        shp = (le - lb, n_seqs, n_kv_heads, -1)
+        shp = (le - lb, n_seqs, n_kv_heads, -1) if n_windows == 1 else (le - lb, n_seqs, n_windows, n_kv_heads, -1)
         out.update(scores=np.stack(sc).reshape(shp), idx_topk=np.stack(it).reshape(shp),
                    idx_final=np.stack(fi).reshape(shp))
     return out

@@ -33,6 +33,7 @@ def chk(oracle):
 
 
 def _parity(gpu, chk, wl, flags_extra=0, overrides=None, lb=None, le=None, use_win_start=True, check_s1=True):
+    NW = wl.shape.n_windows
     kara, gu = gpu
     sh = wl.shape
     p = dict(W=sh.W, U=sh.U, ratio=sh.ratio, alpha=sh.alpha, gamma=sh.gamma)
@@ -45,9 +46,49 @@ def _parity(gpu, chk, wl, flags_extra=0, overrides=None, lb=None, le=None, use_w
     out, cache, _ = gu.gpu_compress(wl, lb, le, flags=flags, use_win_start=use_win_start, overrides=overrides)
     assert out["status"] == 0
     stats = chk.compare(H0, out, sh.n_q_heads, p["W"], p["U"], p["ratio"], p["alpha"], p["gamma"], lb, le,
-                        commit=True, check_s1=check_s1)
+                        commit=True, check_s1=check_s1, n_windows=NW)
     stats["score_path"] = cache.last_score_path()
     return stats, out, H0
+
+
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("NW,S,hist,tail,W,U", [(2, 2, 0, 0, 64, 8), (3, 3, 37, 5, 64, 8), (4, 2, 100, 0, 512, 32),
+                                                (16, 1, 0, 3, 128, 16)])
+def test_prefill_multi_window_call(gpu, chk, NW, S, hist, tail, W, U):
+    """SURVEY 8(f)-1 / PAPER.md App. C.2 (L307): kara_compress_windows — NW disjoint windows per sequence compressed in
+    one call, each window's retained rows + buffer laid down behind those of the window before it (reading G17).
+    Three-stage parity against kara_oracle_compress_windows: scores per (window, head), I, F, every pool byte, block
+    tables, seq_lens and the free list."""
+    big = W >= 512
+    shape = kin.scaled(kin.CFG2 if big else kin.CFG1, n_seqs=S, n_layers=2, n_windows=NW, W=W, U=U,
+                       hist_lo=hist, hist_hi=hist + (40 if hist else 0), tail_lo=tail, tail_hi=tail,
+                       **({} if big else dict(n_q_heads=4, n_kv_heads=2, alpha=4, gamma=4, planted_positions=2)))
+    wl = kin.generate(shape, seed=100 + NW)
+    stats, out, H0 = _parity(gpu, chk, wl)
+    n = W - U
+    keep = stats["keep"]
+    assert stats["units"] == 2 * S * NW * shape.n_kv_heads and stats["score_path"] == 2
+    for s in range(S):
+        h, ln = int(H0["ws"][s]), int(H0["sl"][s])
+        assert out["sl"][s] == h + NW * (keep + U) + (ln - h - NW * W)
+
+
+def test_prefill_one_window_equals_the_decoding_call(gpu, chk):
+    """n_windows = 1 through kara_compress_windows is kara_compress_window bit for bit."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_seqs=3, n_layers=2, hist_lo=20, hist_hi=90), seed=9)
+    sh = wl.shape
+    ref, _, _ = gu.gpu_compress(wl)
+    D = gu.to_cuda(wl)
+    cache = kara.KaraCache(sh.block_size, 2, sh.n_kv_heads, sh.head_dim)
+    cache.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+    cache.compress_windows(0, 2, D["bt"], D["sl"], D["ws"], 1, D["q"], sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma,
+                           kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    out = gu.readback(cache, D, 0, 2, sh.n_seqs, sh.n_kv_heads, kara.KARA_KEEP_DEBUG)
+    for key in ("k", "v", "bt", "sl", "fc", "idx_final", "idx_topk"):
+        np.testing.assert_array_equal(out[key], ref[key], err_msg=key)
+    np.testing.assert_array_equal(out["scores"].view(np.uint32), ref["scores"].view(np.uint32))
 
 
 # ------------------------------------------------------------------------------------------------
