@@ -1,16 +1,22 @@
 #!/usr/bin/env python
 """bench.py — Kara compress_window step on B200: window-compressions/s, KV GB/s, % of roofline.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg3|cfg4|cfg5|cfg1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+                    [--workload cfg4|cfg2|cfg3|cfg5|cfg1|prefill] [--qbuf-only] [--alpha0] [--no-per-config]
 
 A "step" is ONE pass of the whole hot path (a1 score, a2 top-k, a3 Token2Chunk, a4 compaction,
 a5 metadata) over one batch of synthetic input: one kara_compress_window call over all resident
-layers with KARA_COMMIT.  Default workload = BASELINE.json configs[1] (single sequence,
-Qwen3-14B-like 40 layers x 40/8 heads x 128, h=4096, W=512, U=32, r=20 %, alpha=32, gamma=8).
+layers with KARA_COMMIT.  Default workload = BASELINE.json configs[3] (cfg4: 256 concurrent
+sequences, Qwen3-14B-like 40/8 heads x 128, W=1024, U=32, r=20 %, alpha=32, gamma=8, histories in
+[8K, 32K], pool 95 % full; 2 of 40 layers resident — 40 layers do not fit 180 GB), the
+largest single-GPU configuration of the metric.  The same JSON line carries `per_config`: cfg2, cfg3,
+cfg5 and the prefill workload, a few steps each.
 The call is destructive, so between steps the pools / tables / free list are restored from a
 pristine copy and L2 is flushed (both untimed); every step is timed on its own with CUDA events
 on the launching stream, and the K step times are summed (max over ranks for N>1).
 
+`--gpus N` without a torchrun environment starts its N ranks itself (one replica per GPU, no
+data-path collective: DESIGN.md §8) and fails loudly if fewer than N devices are visible.
 Prints ONE JSON line (see DESIGN.md §Measurement for every key).  `--impl reference` times the
 CPU oracle, as it stands, on a bounded sample of the same workload (rank 0 only).
 """
@@ -29,11 +35,14 @@ sys.path.insert(0, str(ROOT))
 
 METRIC = "window-compressions/sec"
 UNIT = "window-compressions/s"
+WORKLOADS = ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "prefill")
+SEEDS = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5, "prefill": 6}
 
 
 def _shape(name):
     from paper_2607_01237_b200 import inputs as kin
-    table = {"cfg1": kin.CFG1, "cfg2": kin.CFG2, "cfg3": kin.CFG3, "cfg4": kin.CFG4, "cfg5": kin.CFG5}
+    table = {"cfg1": kin.CFG1, "cfg2": kin.CFG2, "cfg3": kin.CFG3, "cfg4": kin.CFG4, "cfg5": kin.CFG5,
+             "prefill": kin.PREFILL}
     return table[name]
 
 
@@ -41,12 +50,18 @@ def _resident_layers(name, shape, requested):
     if requested:
         return requested
     # SURVEY §8(d) footprint: cfg 3 fits with all layers only barely, cfg 4/5 do not fit at all
-    return {"cfg3": 8, "cfg4": 2, "cfg5": 8}.get(name, shape.n_layers)
+    return {"cfg3": 8, "cfg4": 2, "cfg5": 8, "prefill": 8}.get(name, shape.n_layers)
+
+
+def _workload_label(name, shape):
+    if name == "prefill":
+        return f"SURVEY 8(f)-1 prefill ({shape.name}: {shape.n_seqs} prompts x {shape.n_windows} windows of {shape.W})"
+    return f"BASELINE.json configs[{int(name[-1]) - 1}] ({shape.name})"
 
 
 def _config(name, shape, L, extra=None):
-    cfg = {"workload": f"BASELINE.json configs[{int(name[-1]) - 1}] ({shape.name})",
-           "n_seqs": shape.n_seqs, "n_layers": L, "n_layers_model": shape.n_layers,
+    cfg = {"workload": _workload_label(name, shape),
+           "n_seqs": shape.n_seqs, "n_windows": shape.n_windows, "n_layers": L, "n_layers_model": shape.n_layers,
            "n_q_heads": shape.n_q_heads, "n_kv_heads": shape.n_kv_heads, "head_dim": shape.head_dim,
            "block_size": shape.block_size, "W": shape.W, "U": shape.U, "retention": shape.ratio,
            "alpha": shape.alpha, "gamma": shape.gamma, "history": [shape.hist_lo, shape.hist_hi],
@@ -58,24 +73,28 @@ def _config(name, shape, L, extra=None):
     return cfg
 
 
-def algorithmic(shape, L):
-    """Algorithmic FLOPs and bytes of one step."""
+def algorithmic(shape, L, qbuf_only=False):
+    """Algorithmic FLOPs and bytes of one step.  A window-compression is
+    one (sequence, layer, window) over all KV heads; with --qbuf-only the queries are the U buffer rows."""
     import math
     n = shape.n
     keep = int(math.ceil(shape.ratio * n - 1e-9))
-    units = shape.n_seqs * L * shape.n_kv_heads
-    flops_unit = 2.0 * shape.W * shape.G * n * shape.head_dim
-    q_bytes = shape.W * shape.G * shape.head_dim * 2
+    units = shape.n_seqs * shape.n_windows * L * shape.n_kv_heads
+    q_rows = shape.U if qbuf_only else shape.W
+    flops_unit = 2.0 * q_rows * shape.G * n * shape.head_dim
+    q_bytes = q_rows * shape.G * shape.head_dim * 2
     k_bytes = n * shape.head_dim * 2
     comp_bytes = 2 * 2 * (keep + shape.U) * shape.head_dim * 2     # K and V, read + write
     return dict(units=units, keep=keep, flops_unit=flops_unit, bytes_unit=q_bytes + k_bytes + comp_bytes,
                 flops=flops_unit * units, bytes=(q_bytes + k_bytes + comp_bytes) * units,
-                kv_in_bytes=shape.n_seqs * L * shape.W * shape.n_kv_heads * shape.head_dim * 2 * 2)
+                score_bytes=(q_bytes + k_bytes) * units,
+                kv_in_bytes=shape.n_seqs * shape.n_windows * L * shape.W * shape.n_kv_heads * shape.head_dim * 2 * 2)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE score-kernel launch from the committed `ncu --set full`
-# capture (profiles/r1_final_ncu_cfg2.md), keyed by (workload, resident layers); None where no capture exists.
-NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40): 257.7e6 + 6.7e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE score-kernel launch, from the committed `ncu --set full`
+# captures of exactly these commands (profiles/r2_ncu_score.md), keyed by (workload, resident layers, variant).
+NCU_SCORE_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_score.md (ncu --set full, dram rd+wr of one score-kernel launch of this workload)"
 
 
 def _peaks():
@@ -137,6 +156,7 @@ class ClockSampler:
 
 
 # -------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline, --impl reference): the oracle as it stands, never tuned for this
 def oracle_prepare(shape, L_sample, seed):
     """Host image of `L_sample` layers of the workload's first sequence for the oracle legs."""
     from oracle import check
@@ -144,8 +164,10 @@ def oracle_prepare(shape, L_sample, seed):
     small = kin.scaled(shape, n_seqs=1, n_layers=L_sample, hist_lo=min(shape.hist_lo, 4096),
                        hist_hi=min(shape.hist_lo, 4096))
     wl = kin.generate(small, seed=seed)
-    desc = (f"{L_sample} layer(s) x 1 sequence x {small.n_kv_heads} KV heads = {L_sample * small.n_kv_heads} units of "
-            f"{shape.name} (whole path O1-O11, fp64, 1 thread); history capped at 4096 tokens (never read)")
+    units = L_sample * small.n_windows * small.n_kv_heads
+    desc = (f"{L_sample} layer(s) x 1 sequence x {small.n_windows} window(s) x {small.n_kv_heads} KV heads = {units} "
+            f"units of {shape.name} (whole path O1-O11, fp64, 1 thread per process); history capped at 4096 tokens "
+            f"(never read)")
     return small, check.host_image(wl), desc
 
 
@@ -154,8 +176,43 @@ def oracle_leg(small, H, L_sample):
     from oracle import check
     Hc = {k: v.copy() for k, v in H.items()}
     t0 = time.perf_counter()
-    check.run_oracle(Hc, small.n_q_heads, small.W, small.U, small.ratio, small.alpha, small.gamma, 0, L_sample)
+    check.run_oracle(Hc, small.n_q_heads, small.W, small.U, small.ratio, small.alpha, small.gamma, 0, L_sample,
+                     n_windows=small.n_windows)
     return time.perf_counter() - t0
+
+
+def _oracle_worker(args):
+    """One process of the all-cores leg: its own sample (a different seed per process), a barrier so that all
+    processes run the oracle at the same time, then one timed pass.  Returns (start, end) wall-clock stamps."""
+    workload, L_sample, seed, barrier = args
+    sys.path.insert(0, str(ROOT))
+    small, H, _ = oracle_prepare(_shape(workload), L_sample, seed)
+    from oracle import check
+    barrier.wait()
+    t0 = time.time()
+    check.run_oracle(H, small.n_q_heads, small.W, small.U, small.ratio, small.alpha, small.gamma, 0, L_sample,
+                     n_windows=small.n_windows)
+    return t0, time.time()
+
+
+def oracle_all_cores(workload, L_per_proc):
+    """Independent units in one worker process per core of sched_getaffinity (process-level parallelism, no shared
+    code with the GPU path): window-compressions of all processes / (last end - first start)."""
+    import multiprocessing as mp
+    cores = len(os.sched_getaffinity(0))
+    ctx = mp.get_context("spawn")
+    with ctx.Manager() as mgr:
+        barrier = mgr.Barrier(cores)
+        with ctx.Pool(cores) as pool:
+            stamps = pool.map(_oracle_worker, [(workload, L_per_proc, 100 + i, barrier) for i in range(cores)])
+    wall = max(e for _, e in stamps) - min(s for s, _ in stamps)
+    shape = _shape(workload)
+    return cores, cores * L_per_proc * shape.n_windows / wall, wall
+
+
+# layers of one sequence per oracle pass: about 10-30 s of CPU work on one core
+ORACLE_LAYERS = {"cfg1": 1, "cfg2": 24, "cfg3": 24, "cfg4": 6, "cfg5": 2, "prefill": 2}
+ORACLE_LAYERS_PER_PROC = {"cfg1": 1, "cfg2": 8, "cfg3": 8, "cfg4": 2, "cfg5": 1, "prefill": 1}
 
 
 def run_reference(args):
@@ -163,13 +220,13 @@ def run_reference(args):
     if rank != 0:
         return
     shape = _shape(args.workload)
-    L_sample = 1     # one layer of one sequence per step (cfg 2: 8 units, about 1.2 s)
+    L_sample = 1     # one layer of one sequence per step (cfg 4: 8 units, about 2 s)
     small, H, desc = oracle_prepare(shape, L_sample, seed=2)
     for _ in range(args.warmup):
         oracle_leg(small, H, L_sample)
     times = [oracle_leg(small, H, L_sample) for _ in range(args.steps)]
     total = sum(times)
-    value = L_sample * args.steps / total
+    value = L_sample * small.n_windows * args.steps / total
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -181,35 +238,28 @@ def run_reference(args):
 
 
 # -------------------------------------------------------------------------------------------------
-def run_gpu(args):
+def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False, qbuf_only=False, alpha0=False,
+            score_timing=True, want_e2e=False):
+    """Generates workload `name` on `dev`, times `steps` steps (after `warmup`) and returns the raw numbers."""
     import torch
     from paper_2607_01237_b200 import inputs as kin
     from paper_2607_01237_b200 import kara
     from paper_2607_01237_b200 import replicas
 
-    rank, local_rank, world = replicas.rank_env()
-    dist = None
-    if world > 1:
-        import torch.distributed as dist_mod
-        dist = dist_mod
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
-    torch.cuda.set_device(local_rank)
-    dev = torch.device(f"cuda:{local_rank}")
-    kara.lib()
-
-    shape = _shape(args.workload)
-    L = _resident_layers(args.workload, shape, args.layers)
-    seed = replicas.rank_seed({"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}[args.workload], rank)
-    fill = "randn" if args.workload in ("cfg1", "cfg2") else "pattern"
+    shape = _shape(name)
+    if alpha0:
+        shape = kin.scaled(shape, alpha=0)                   # "w/o Token2Chunk" (PAPER.md:L195)
+    L = _resident_layers(name, shape, L_req)
+    NW = shape.n_windows
+    seed = replicas.rank_seed(SEEDS[name], rank)
+    fill = "randn" if name in ("cfg1", "cfg2") else "pattern"
     wl = kin.generate(shape, seed=seed, device=dev, n_layers_resident=L, history_fill=fill)
-    alg = algorithmic(shape, L)
-    peaks = _peaks()
 
     cache = kara.KaraCache(shape.block_size, L, shape.n_kv_heads, shape.head_dim)
     cache.attach_pool(wl.k_pool, wl.v_pool, wl.free_list, wl.free_count)
-    cache.enable_score_timing(not args.no_score_timing)
-    flags = kara.KARA_COMMIT | (kara.KARA_SCORE_SIMT if args.simt else 0)
-    ws = torch.empty(cache.workspace_bytes(L, shape.n_seqs, shape.n_q_heads, shape.W, shape.U, shape.ratio,
+    cache.enable_score_timing(score_timing)
+    flags = kara.KARA_COMMIT | (kara.KARA_SCORE_SIMT if simt else 0) | (kara.KARA_SCORE_QBUF_ONLY if qbuf_only else 0)
+    ws = torch.empty(cache.workspace_bytes(L, shape.n_seqs * NW, shape.n_q_heads, shape.W, shape.U, shape.ratio,
                                            shape.alpha), dtype=torch.uint8, device=dev)
     # pristine copies: only the window blocks change, but a full copy is simple and untimed
     if wl.k_pool.numel() * 2 <= 8 << 30:
@@ -236,22 +286,31 @@ def run_gpu(args):
         torch.cuda.synchronize()
 
     def step():
-        cache.compress_window(0, L, wl.block_table, wl.seq_lens, wl.win_start, wl.window_q, shape.W, shape.U,
-                              shape.ratio, shape.alpha, shape.gamma, flags, workspace=ws)
+        if NW > 1:
+            cache.compress_windows(0, L, wl.block_table, wl.seq_lens, wl.win_start, NW, wl.window_q, shape.W, shape.U,
+                                   shape.ratio, shape.alpha, shape.gamma, flags, workspace=ws)
+        else:
+            cache.compress_window(0, L, wl.block_table, wl.seq_lens, wl.win_start, wl.window_q, shape.W, shape.U,
+                                  shape.ratio, shape.alpha, shape.gamma, flags, workspace=ws)
 
     stream = torch.cuda.current_stream(dev)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         restore(); step(); torch.cuda.synchronize()
     assert cache.status() == 0, "device status word set during warm-up"
     freed = int(wl.free_count[0]) - int(fc0[0])
+    score_path = cache.last_score_path()
+    if score_path != 2 and not simt:
+        # north_star: no multi-backend dispatch — a bench number from the CUDA-core kernel is not a bench number
+        raise SystemExit(f"bench.py: workload {name} did not run on the tcgen05/TMA score kernel "
+                         f"(kara_last_score_path = {score_path}); pass --simt to time the CUDA-core kernel on purpose")
 
     step_ms, score_ms = [], []
     if dist:
         dist.barrier()
     torch.cuda.synchronize()
     with ClockSampler(local_rank) as clk:
-        for _ in range(args.steps):
+        for _ in range(steps):
             restore()
             ev0.record(stream); step(); ev1.record(stream)
             torch.cuda.synchronize()
@@ -260,71 +319,137 @@ def run_gpu(args):
     if dist:
         dist.barrier()
     torch.cuda.synchronize()
-    launches = cache.last_launch_count() * args.steps
-    score_path = cache.last_score_path()
-    total_ms = sum(step_ms)
+    res = dict(shape=shape, L=L, total_ms=sum(step_ms), score_ms=sum(score_ms) / len(score_ms), freed=freed,
+               launches=cache.last_launch_count() * steps, score_path=score_path, clocks=clk.summary(),
+               alg=algorithmic(shape, L, qbuf_only), wc_step=shape.n_seqs * NW * L, e2e=None)
 
     # ---- e2e: same step through the host-buffer entry point (pinned host inputs) -------------
-    hq = wl.window_q.cpu().pin_memory()
-    hbt, hsl, hws = bt0.cpu().pin_memory(), sl0.cpu().pin_memory(), wl.win_start.cpu().pin_memory()
-    h2d = hq.numel() * 2 + hbt.numel() * 4 + hsl.numel() * 4 + hws.numel() * 4
-    d2h = hbt.numel() * 4 + hsl.numel() * 4 + 4
-    e2e_s = []
-    n_e2e = max(3, min(args.steps, 10))
-    for it in range(2 + n_e2e):
-        restore()
-        hbt.copy_(bt0.cpu()); hsl.copy_(sl0.cpu())
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        cache.compress_window_host(0, L, hbt, hsl, hws, hq, shape.W, shape.U, shape.ratio, shape.alpha, shape.gamma,
-                                   flags)
-        dt = time.perf_counter() - t0
-        if it >= 2:
-            e2e_s.append(dt)
-    e2e_total = sum(e2e_s)
+    if want_e2e and NW == 1:
+        hq = wl.window_q.cpu().pin_memory()
+        hbt, hsl, hws = bt0.cpu().pin_memory(), sl0.cpu().pin_memory(), wl.win_start.cpu().pin_memory()
+        h2d = hq.numel() * 2 + hbt.numel() * 4 + hsl.numel() * 4 + hws.numel() * 4
+        d2h = hbt.numel() * 4 + hsl.numel() * 4 + 4
+        e2e_s = []
+        n_e2e = max(3, min(steps, 10))
+        for it in range(2 + n_e2e):
+            restore()
+            hbt.copy_(bt0.cpu()); hsl.copy_(sl0.cpu())
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            cache.compress_window_host(0, L, hbt, hsl, hws, hq, shape.W, shape.U, shape.ratio, shape.alpha, shape.gamma,
+                                       flags)
+            dt = time.perf_counter() - t0
+            if it >= 2:
+                e2e_s.append(dt)
+        res["e2e"] = dict(mean_s=sum(e2e_s) / len(e2e_s), h2d=h2d, d2h=d2h)
+        del hq
+    cache.close()
+    del wl, k0, v0, ws, flush, cache
+    torch.cuda.empty_cache()
+    return res
 
-    total_ms, e2e_mean = replicas.max_over_ranks([total_ms, e2e_total / len(e2e_s)], dist, dev)
 
-    wc_step = shape.n_seqs * L                      # window-compressions per step per GPU
-    value = replicas.job_throughput(world, wc_step, args.steps, total_ms)
-    ms_per_step = total_ms / args.steps
-    sc_ms = sum(score_ms) / len(score_ms)
+def derived(res, peaks, world=1, total_ms=None, steps=1):
+    """Throughput and roofline figures of one measure() result (total_ms: max over ranks if given)."""
+    alg = res["alg"]
+    ms_per_step = (total_ms if total_ms is not None else res["total_ms"]) / steps
+    sc_ms = res["score_ms"]
     t_tensor_ms = alg["flops"] / (peaks["bf16_tflops"] * 1e12) * 1e3
     t_hbm_ms = alg["bytes"] / (peaks["hbm_gbs"] * 1e9) * 1e3
-    achieved_tflops = alg["flops"] / (sc_ms * 1e-3) / 1e12
+    return dict(ms_per_step=ms_per_step, value=world * res["wc_step"] / (ms_per_step * 1e-3),
+                kv_gbs=world * alg["kv_in_bytes"] / (ms_per_step * 1e-3) / 1e9,
+                algorithmic_gbs=world * alg["bytes"] / (ms_per_step * 1e-3) / 1e9,
+                step_tflops=world * alg["flops"] / (ms_per_step * 1e-3) / 1e12,
+                score_ms=sc_ms, score_tflops=alg["flops"] / (sc_ms * 1e-3) / 1e12 if sc_ms > 0 else None,
+                score_gbs=alg["score_bytes"] / (sc_ms * 1e-3) / 1e9 if sc_ms > 0 else None,
+                t_tensor_ms=t_tensor_ms, t_hbm_ms=t_hbm_ms, step_frac=max(t_tensor_ms, t_hbm_ms) / ms_per_step)
 
+
+# -------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    from paper_2607_01237_b200 import kara
+    from paper_2607_01237_b200 import replicas
+
+    rank, local_rank, world = replicas.rank_env()
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    replicas.require_devices(world if world > 1 else 1, torch.cuda.device_count())
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device(f"cuda:{local_rank}")
+    kara.lib()
+    peaks = _peaks()
+    variant = "qbuf_only" if args.qbuf_only else "alpha0" if args.alpha0 else "full"
+
+    res = measure(args.workload, args.layers, args.steps, args.warmup, dev, rank, dist, local_rank, simt=args.simt,
+                  qbuf_only=args.qbuf_only, alpha0=args.alpha0, score_timing=not args.no_score_timing, want_e2e=True)
+    e2e_mean = res["e2e"]["mean_s"] if res["e2e"] else 0.0
+    total_ms, e2e_mean = replicas.max_over_ranks([res["total_ms"], e2e_mean], dist, dev)
+    shape, L, alg = res["shape"], res["L"], res["alg"]
+    d = derived(res, peaks, world, total_ms, args.steps)
+
+    if args.qbuf_only:
+        # "w/o Bi-Attention" (PAPER.md:L193): U x n logits per head — 16 x fewer FLOPs at the same K bytes: HBM-bound
+        roofline = {"kernel": "score (a1), buffer queries only", "bound": "hbm", "achieved": d["score_gbs"],
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": d["score_gbs"] / peaks["hbm_gbs"] if d["score_gbs"] else None,
+                    "bytes_per_launch": alg["score_bytes"]}
+    else:
+        roofline = {"kernel": "score (a1)", "bound": "tensor", "achieved": d["score_tflops"],
+                    "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                    "frac": d["score_tflops"] / peaks["bf16_tflops"] if d["score_tflops"] else None,
+                    "flops_per_launch": alg["flops"]}
+    roofline.update({"traffic": NCU_SCORE_TRAFFIC_BYTES.get((args.workload, L, variant)),
+                     "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peaks["source"] + ", burst",
+                     "kernel_ms": d["score_ms"], "share_of_step": d["score_ms"] / d["ms_per_step"]})
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": d["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": d["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": _config(args.workload, shape, L, {"score_kernel": {1: "simt", 2: "tcgen05+tma"}.get(score_path),
-                                                     "freed_blocks_per_step": freed}),
-        "kv_gbs": world * alg["kv_in_bytes"] / (ms_per_step * 1e-3) / 1e9,
-        "algorithmic_gbs": world * alg["bytes"] / (ms_per_step * 1e-3) / 1e9,
-        "step_tflops": world * alg["flops"] / (ms_per_step * 1e-3) / 1e12,
-        "clocks": clk.summary(),
-        "e2e": {"value": world * wc_step / e2e_mean, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_mean * 1e3,
-                "api": "kara_compress_window_host (pinned host window_q/tables in, tables + free count out)"},
-        "gpu_launches": launches,
-        "roofline": {"kernel": "score (a1)", "bound": "tensor", "achieved": achieved_tflops,
-                     "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": achieved_tflops / peaks["bf16_tflops"],
-                     "traffic": NCU_SCORE_TRAFFIC_BYTES.get((args.workload, L)),
-                     "traffic_source": "profiles/r1_final_ncu_cfg2.md (ncu --set full, dram rd+wr of one launch)",
-                     "peak_source": peaks["source"] + ", burst bf16", "kernel_ms": sc_ms,
-                     "flops_per_launch": alg["flops"], "share_of_step": sc_ms / ms_per_step},
-        "step_roofline": {"t_tensor_ms": t_tensor_ms, "t_hbm_ms": t_hbm_ms,
-                          "frac": max(t_tensor_ms, t_hbm_ms) / ms_per_step,
+        "config": _config(args.workload, shape, L, {"score_kernel": {1: "simt", 2: "tcgen05+tma"}.get(res["score_path"]),
+                                                     "variant": variant, "freed_blocks_per_step": res["freed"]}),
+        "kv_gbs": d["kv_gbs"], "algorithmic_gbs": d["algorithmic_gbs"], "step_tflops": d["step_tflops"],
+        "clocks": res["clocks"],
+        "e2e": ({"value": world * res["wc_step"] / e2e_mean, "unit": UNIT, "h2d_bytes_per_step": res["e2e"]["h2d"],
+                 "d2h_bytes_per_step": res["e2e"]["d2h"], "ms_per_step": e2e_mean * 1e3,
+                 "api": "kara_compress_window_host (pinned host window_q/tables in, tables + free count out)"}
+                if res["e2e"] else None),
+        "gpu_launches": res["launches"],
+        "roofline": roofline,
+        "step_roofline": {"t_tensor_ms": d["t_tensor_ms"], "t_hbm_ms": d["t_hbm_ms"], "frac": d["step_frac"],
                           "def": "slower of (algorithmic bytes / measured HBM GB/s) and (score FLOPs / measured bf16 TFLOP/s) over ms_per_step"},
     }
+    if rank == 0 and world == 1 and not args.no_per_config:
+        # the other configs of BASELINE.json (and the prefill workload), a few steps each, same protocol
+        per = {}
+        for name in ("cfg2", "cfg3", "cfg5", "prefill"):
+            if name == args.workload:
+                continue
+            r = measure(name, 0, 5, 3, dev, rank, None, local_rank)
+            dd = derived(r, peaks, 1, None, 5)
+            per[name] = {"workload": _workload_label(name, r["shape"]), "n_layers": r["L"], "steps": 5,
+                         "ms_per_step": dd["ms_per_step"], "value": dd["value"], "kv_gbs": dd["kv_gbs"],
+                         "roofline_frac": dd["score_tflops"] / peaks["bf16_tflops"], "score_kernel_ms": dd["score_ms"],
+                         "step_roofline_frac": dd["step_frac"], "freed_blocks_per_step": r["freed"],
+                         "gpu_launches": r["launches"], "sm_mhz": r["clocks"]["sm_mhz"]}
+        line["per_config"] = per
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
-            Ls = {"cfg1": 1, "cfg2": 24, "cfg3": 24, "cfg4": 6, "cfg5": 2}[args.workload]   # ~10-30 s of CPU work
+            Ls = ORACLE_LAYERS[args.workload]
             small, H, desc = oracle_prepare(shape, Ls, seed=2)
             secs = oracle_leg(small, H, Ls)
-            import multiprocessing
-            line["cpu_baseline"] = {"value": Ls / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
-                                    "seconds": secs, "host_cores_available": multiprocessing.cpu_count()}
+            line["cpu_baseline"] = {"value": Ls * small.n_windows / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": desc, "seconds": secs}
+            cores, v_all, wall = oracle_all_cores(args.workload, ORACLE_LAYERS_PER_PROC[args.workload])
+            line["cpu_baseline"]["all_cores"] = {
+                "value": v_all, "unit": UNIT, "cores": cores, "seconds": wall,
+                "how": f"{cores} worker processes (one per core of sched_getaffinity), each the single-threaded oracle on "
+                       f"{ORACLE_LAYERS_PER_PROC[args.workload]} layer(s) of its own sequence, started together"}
         print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
@@ -336,16 +461,26 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg4", choices=list(WORKLOADS))
     ap.add_argument("--layers", type=int, default=0, help="resident layers (default: all that fit)")
     ap.add_argument("--simt", action="store_true", help="force the CUDA-core score kernel")
+    ap.add_argument("--qbuf-only", action="store_true",
+                    help="ablation 'w/o Bi-Attention' (PAPER.md:L193): score with the buffer's queries only (HBM-bound)")
+    ap.add_argument("--alpha0", action="store_true", help="ablation 'w/o Token2Chunk' (PAPER.md:L195): alpha = 0")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config legs (cfg2, cfg3, cfg5, prefill)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-score-timing", action="store_true",
                     help="no CUDA events inside the library around the score launch (roofline.kernel_ms = 0)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    from paper_2607_01237_b200 import replicas
     if args.impl == "reference":
         run_reference(args)
+    elif replicas.needs_spawn(args.gpus):
+        # started plainly with --gpus N: start the N ranks (one replica per GPU) and let rank 0 print the line
+        import torch
+        replicas.require_devices(args.gpus, torch.cuda.device_count())
+        sys.exit(replicas.spawn_ranks(args.gpus, [str(Path(__file__).resolve()), *sys.argv[1:]]))
     else:
         run_gpu(args)
 

@@ -59,3 +59,36 @@ def test_single_process_is_identity():
     assert replicas.max_over_ranks([1.5, 2.5]) == [1.5, 2.5]
     assert replicas.rank_seed(2, 0) == 2 and replicas.rank_seed(2, 3) == 3002
     assert replicas.job_throughput(1, 40, 10, 2.0) == 40 * 10 / 2e-3
+
+
+def test_bench_launcher_starts_n_ranks():
+    """`bench.py --gpus N` started plainly must start its N ranks itself (replicas.needs_spawn / spawn_ranks): the
+    launcher re-executes the script under torch.distributed.run; here with a CPU stand-in for the step (gloo)."""
+    import json
+    from paper_2607_01237_b200 import replicas
+    env_had = os.environ.pop("WORLD_SIZE", None)
+    try:
+        assert replicas.needs_spawn(2) and not replicas.needs_spawn(1)
+        rc, out = replicas.spawn_ranks(2, [str(ROOT / "tests" / "replica_step_cpu.py"), "3"], capture=True)
+    finally:
+        if env_had is not None:
+            os.environ["WORLD_SIZE"] = env_had
+    assert rc == 0
+    lines = [json.loads(x) for x in out.splitlines() if x.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["steps"] == 3 and lines[0]["value"] > 0
+
+
+def test_bench_gpus_n_without_devices_fails_loudly():
+    """Fewer CUDA devices than ranks is an error, never a silent N = 1 run."""
+    import subprocess
+    import pytest
+    import torch
+    from paper_2607_01237_b200 import replicas
+    with pytest.raises(SystemExit):
+        replicas.require_devices(2, 1)
+    replicas.require_devices(2, 2)
+    if torch.cuda.device_count() < 2:
+        env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+        r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--gpus", "2", "--steps", "1"], env=env,
+                           capture_output=True, text=True)
+        assert r.returncode != 0 and "only" in r.stderr and "--gpus 2" in r.stderr
