@@ -396,7 +396,9 @@ def test_cfg2_full_size_sampled_units(gpu, oracle):
         if not np.array_equal(F, own["F"]):
             assert check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 hard mismatch at unit {(l, hk)}"
             n_amb += 1
-    assert n_amb <= len(sample)
+    # S3 exceptions are only ever excused by a measured near-tie (asserted above); report the fraction
+    print(f"cfg2 full size: {n_amb} of {len(sample)} sampled units ambiguous (near-tie < 1e-3 at a decision boundary)")
+    assert n_amb <= len(sample) // 2, "more than half of the sampled units differ from the oracle at near-ties"
 
 
 def test_scores_are_bit_reproducible_run_to_run(gpu):
@@ -424,7 +426,8 @@ def test_odd_shapes_against_the_oracle(gpu, chk, W, U, d, G, bs, hist):
     assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
 
 
-@pytest.mark.parametrize("name,L,ratio", [("cfg3", 2, 0.2), ("cfg4", 1, 0.1), ("cfg4", 1, 0.3), ("cfg5", 1, 0.2)])
+@pytest.mark.parametrize("name,L,ratio", [("cfg3", 2, 0.2), ("cfg4", 1, 0.1), ("cfg4", 1, 0.2), ("cfg4", 1, 0.3),
+                                          ("cfg5", 1, 0.2)])
 def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
     """BASELINE.json configs[2..4] at their batch sizes, in the launch configuration bench.py times (generated on
     the device, L resident layers): cfg3 = 64 sequences, histories in [2K, 16K] (not block aligned), block tables
@@ -441,6 +444,7 @@ def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
     S, Hkv, G, n, bs = sh.n_seqs, sh.n_kv_heads, sh.n_q_heads // sh.n_kv_heads, sh.W - sh.U, sh.block_size
     k0, v0 = wl.k_pool.clone(), wl.v_pool.clone()
     bt0, sl0, fc0 = wl.block_table.clone(), wl.seq_lens.clone(), int(wl.free_count[0])
+    fl0 = wl.free_list.clone()
     cache = kara.KaraCache(bs, L, Hkv, sh.head_dim)
     cache.attach_pool(wl.k_pool, wl.v_pool, wl.free_list, wl.free_count)
     cache.compress_window(0, L, wl.block_table, wl.seq_lens, wl.win_start, wl.window_q, sh.W, sh.U, sh.ratio,
@@ -467,10 +471,27 @@ def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
         F = cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, s, hk)
         assert abs(float(A.astype(np.float64).sum()) - G * sh.W) <= 1e-4 * G * sh.W
         assert F.shape[0] == keep and np.all(np.diff(F) > 0) and F[0] >= 0 and F[-1] < n
-    # sampled units against the oracle
+    # a5 on the WHOLE batch: the oracle's metadata step on the pristine tables -> block tables, seq_lens and the free list
+    # (order included) must be bit-identical
+    bt_o, sl_o = bt0.cpu().numpy().copy(), sl0.cpu().numpy().copy()
+    fl_o, fc_o = fl0.cpu().numpy().copy(), np.array([fc0], np.int32)
+    ko.metadata(bt_o, sl_o, wl.win_start.cpu().numpy().copy(), bs, sh.W, sh.U, keep, fl_o, fc_o)
+    np.testing.assert_array_equal(wl.block_table.cpu().numpy(), bt_o)
+    np.testing.assert_array_equal(wl.seq_lens.cpu().numpy(), sl_o)
+    assert int(wl.free_count[0]) == int(fc_o[0])
+    np.testing.assert_array_equal(wl.free_list.cpu().numpy()[: int(fc_o[0])], fl_o[: int(fc_o[0])])
+    # sampled units against the oracle: sequences across the history-length deciles plus the sequences that own the
+    # lowest and the highest block id of the pool (both pool ends), layers / heads drawn at random
     rng = np.random.default_rng(11)
-    for _ in range(6 if name != "cfg5" else 2):          # (a cfg5 unit is 8.3 GFLOP for the oracle)
-        l, s, hk = int(rng.integers(L)), int(rng.integers(S)), int(rng.integers(Hkv))
+    n_samples = 4 if name == "cfg5" else 16                # (a cfg5 unit is 8.3 GFLOP for the oracle)
+    order = np.argsort(h, kind="stable")
+    picks = [int(order[min(S - 1, (d * S) // max(n_samples - 2, 1))]) for d in range(n_samples - 2)]
+    bt_np = bt0.cpu().numpy()
+    live = np.where(bt_np >= 0, bt_np, np.iinfo(np.int32).max)
+    picks += [int(np.argmin(live.min(axis=1))), int(np.argmax(np.where(bt_np >= 0, bt_np, -1).max(axis=1)))]
+    n_amb = 0
+    for s in picks:
+        l, hk = int(rng.integers(L)), int(rng.integers(Hkv))
         hs, ols, ts = int(h[s]), int(old_len[s]), int(t[s])
         q_bits = check.bits(wl.window_q[l, s, :, hk * G:(hk + 1) * G, :])
         k_old = check.bits(kin.logical_rows(k0, l, bt0[s], ols, hk))
@@ -484,4 +505,64 @@ def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
             got = cache.gather_debug(what, l, s, hk, wl.block_table, wl.seq_lens)
             np.testing.assert_array_equal(got, ko.compact_rows(old, hs, sh.W, sh.U, ts, F))
         own = ko.select(A32, keep, sh.alpha, sh.gamma)["F"]                                   # S3
-        assert np.array_equal(F, own) or check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 {(l, s, hk)}"
+        if not np.array_equal(F, own):
+            assert check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 {(l, s, hk)}"
+            n_amb += 1
+    print(f"{name} r={ratio}: {n_amb} of {len(picks)} sampled units ambiguous (near-tie < 1e-3 at a decision boundary)")
+
+
+@pytest.mark.parametrize("bs,W,U,d,G,hist", [(128, 512, 32, 128, 5, 300), (256, 768, 32, 128, 4, 1000), (256, 320, 16, 64, 2, 77),
+                                             (128, 1024, 32, 128, 2, 5)])
+def test_large_block_sizes(gpu, chk, bs, W, U, d, G, hist):
+    """include/kara.h admits block sizes up to 256; the paper's own KvLLM setting is block 256 with W = 768 = 3 blocks,
+    U = 32.  Block sizes 128 / 256 put 2 / 1 blocks into a CTA's 256-row key panel; windows start
+    anywhere inside a block.  Full three-stage parity."""
+    shape = kin.scaled(kin.CFG2, n_seqs=3, n_layers=2, n_q_heads=2 * G, n_kv_heads=2, head_dim=d, block_size=bs,
+                       W=W, U=U, alpha=16, gamma=8, hist_lo=hist, hist_hi=hist + 2 * bs + 7, tail_lo=0, tail_hi=bs - 1)
+    stats, _, _ = _parity(gpu, chk, kin.generate(shape, seed=bs + W))
+    assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
+
+
+@pytest.mark.parametrize("shape_name", ["cfg2", "cfg4"])
+def test_buffer_only_queries_full_parity(gpu, oracle, shape_name):
+    """KARA_SCORE_QBUF_ONLY ('w/o Bi-Attention') at the cfg2 / cfg4 shapes: the U = 32 buffer rows are the
+    last quarter of a 128-row tile, d = 128, clusters of 2 / 4 CTAs.  S1: scores against kara_oracle_scores_buffer_queries on
+    every unit; S2: the oracle's O4-O11 re-run on the GPU's scores -> I, F, pools, tables, free list bit-identical; S3: GPU F
+    against the oracle's F from its own buffer-query scores unless a decision boundary is a near-tie."""
+    kara, gu = gpu
+    from oracle import check
+    from oracle import kara_oracle as ko
+    base = kin.CFG2 if shape_name == "cfg2" else kin.CFG4
+    shape = kin.scaled(base, n_seqs=2, n_layers=2, hist_lo=130, hist_hi=700, pool_slack=1.2)
+    wl = kin.generate(shape, seed=41)
+    sh = wl.shape
+    H0 = check.host_image(wl)
+    out, cache, _ = gu.gpu_compress(wl, flags=kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG | kara.KARA_SCORE_QBUF_ONLY)
+    assert out["status"] == 0 and cache.last_score_path() == 2
+    n, G, bs = sh.n, sh.G, sh.block_size
+    keep = ko.budget(n, sh.ratio)
+    n_amb = 0
+    for l in range(2):
+        for s in range(sh.n_seqs):
+            h = int(H0["ws"][s])
+            pos = np.arange(h, h + n)
+            for hk in range(sh.n_kv_heads):
+                krows = np.ascontiguousarray(H0["k"][l, H0["bt"][s, pos // bs], hk, pos % bs])
+                q = np.ascontiguousarray(H0["q"][l, s][:, hk * G:(hk + 1) * G])
+                A64, A32 = ko.scores(q, krows, buffer_only_U=sh.U)
+                A = out["scores"][l, s, hk]
+                assert (np.abs(A - A64) <= check.score_tolerance(A64, G, sh.U, n)).all(), f"S1 {(l, s, hk)}"   # S1
+                own = ko.select(A32, keep, sh.alpha, sh.gamma)["F"]                                        # S3
+                if not np.array_equal(out["idx_final"][l, s, hk], own):
+                    assert check.is_ambiguous(A32, keep, sh.alpha, sh.gamma), f"S3 {(l, s, hk)}"
+                    n_amb += 1
+    Hs = {k_: v_.copy() for k_, v_ in H0.items()}                                                           # S2
+    inj = check.run_oracle(Hs, sh.n_q_heads, sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma, 0, 2, True,
+                           scores_in=np.ascontiguousarray(out["scores"], np.float32))
+    np.testing.assert_array_equal(out["idx_topk"], inj["idx_topk"])
+    np.testing.assert_array_equal(out["idx_final"], inj["idx_final"])
+    for key in ("k", "v", "bt", "sl", "fc"):
+        np.testing.assert_array_equal(out[key], Hs[key], err_msg=key)
+    nfree = int(Hs["fc"][0])
+    np.testing.assert_array_equal(out["fl"][:nfree], Hs["fl"][:nfree])
+    print(f"qbuf-only {shape_name}: {n_amb} of {2 * sh.n_seqs * sh.n_kv_heads} units ambiguous")
