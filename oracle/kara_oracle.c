@@ -427,3 +427,69 @@ done:
   free(kwin); free(A32); free(I); free(F); free(tmp);
   return rc;
 }
+
+/* ---------------------------------------------------------------------------------------- */
+/* Alg. 1 (reading G12) + App. C.4 (L352-354): one decoding step of the periodic policy. */
+int kara_oracle_policy_step(int n_seqs, int max_blocks, int block_size, int32_t* block_table, int32_t* seq_lens,
+                            int32_t* uncompressed, const uint8_t* active, int32_t* free_list, int32_t* free_count,
+                            int32_t* step_counter, int delta, int W, int max_select,
+                            int32_t* sel_ids, int32_t* sel_count, int32_t* sel_block_table, int32_t* sel_seq_lens,
+                            int32_t* sel_win_start, int32_t* exhausted) {
+  if (n_seqs < 0 || max_blocks <= 0 || block_size <= 0 || delta <= 0 || W <= 0 || max_select < 0)
+    return KARA_ORACLE_EINVAL;
+  /* l.2: one generated token per active sequence */
+  for (int s = 0; s < n_seqs; ++s) {
+    if (active && !active[s]) continue;
+    const int len = seq_lens[s];
+    if (len % block_size == 0) {                       /* the token opens a new block */
+      const int b = len / block_size;
+      if (b >= max_blocks || *free_count <= 0) { if (exhausted) ++*exhausted; continue; }
+      block_table[(long)s * max_blocks + b] = free_list[--*free_count];      /* pop from the top of the stack */
+    }
+    seq_lens[s] = len + 1;
+    uncompressed[s] += 1;
+  }
+  /* l.3 */
+  *step_counter += 1;
+  const int g = *step_counter;
+  /* l.4-5 */
+  int cnt = 0;
+  if (g > W && g % delta == 0) {
+    for (int s = 0; s < n_seqs && cnt < max_select; ++s) {
+      if (active && !active[s]) continue;
+      const int len = seq_lens[s];
+      const int t = len % block_size;                  /* the last (possibly partial) block is excluded */
+      if (uncompressed[s] - t < W) continue;
+      sel_ids[cnt] = s;
+      sel_win_start[cnt] = len - t - W;
+      sel_seq_lens[cnt] = len;
+      memcpy(sel_block_table + (long)cnt * max_blocks, block_table + (long)s * max_blocks,
+             sizeof(int32_t) * (size_t)max_blocks);
+      ++cnt;
+    }
+  }
+  for (int x = cnt; x < max_select; ++x) {
+    sel_ids[x] = -1;
+    sel_seq_lens[x] = -1;
+    sel_win_start[x] = 0;
+    for (int b = 0; b < max_blocks; ++b) sel_block_table[(long)x * max_blocks + b] = -1;
+  }
+  *sel_count = cnt;
+  return KARA_ORACLE_OK;
+}
+
+/* Alg. 1 l.12 UpdateMetadata(e) for the running queue + the uncompressed-tail counter of App. C.4 (L354). */
+int kara_oracle_policy_commit(int max_blocks, const int32_t* sel_ids, int sel_count, const int32_t* sel_block_table,
+                              const int32_t* sel_seq_lens, const int32_t* sel_win_start, int keep, int U,
+                              int32_t* block_table, int32_t* seq_lens, int32_t* uncompressed) {
+  for (int x = 0; x < sel_count; ++x) {
+    const int s = sel_ids[x];
+    if (s < 0) return KARA_ORACLE_EINVAL;
+    memcpy(block_table + (long)s * max_blocks, sel_block_table + (long)x * max_blocks,
+           sizeof(int32_t) * (size_t)max_blocks);
+    seq_lens[s] = sel_seq_lens[x];
+    const int t = sel_seq_lens[x] - (sel_win_start[x] + keep + U);
+    uncompressed[s] = U + t;
+  }
+  return KARA_ORACLE_OK;
+}

@@ -17,12 +17,13 @@
  *   Sec 4.3 / Alg. 1 l.11-12 / App. C.4 compaction + block release
  * No blocking, fusion or reordering beyond what those passages state.  Readings of the
  * places where the paper is silent (GQA sum, tie-breaks, rounding of ceil(r n), order of
- * retained rows, free-list order) are the ones listed in DESIGN.md "Readings" (G1..G16).
+ * retained rows, free-list order, prefill windows, policy order) are the ones listed in DESIGN.md "Readings" (G1..G18).
  *
  * Pins (tests/test_oracle_*.py): library float64 softmax on small cases, closed forms
  * (Q = 0, equal keys, one-hot), invariants (sum_j A_j = G*W), equivariances, integer
  * budget table, brute-force Token2Chunk on tiny n, hand-worked vectors under tests/golden/,
- * closed-form freed-block counts.  End-to-end against outputs printed by the paper:
+ * closed-form freed-block counts; the policy step against a token-level simulation (every token carries its own
+ * "compressed" flag) and the paper's KvLLM numbers (B.1).  End-to-end against outputs printed by the paper:
  * PARITY UNPINNED — the paper prints no scores, indices or bytes for any input.
  *
  * Notation (window-relative, 0-based): W window length, U protected buffer at the window's
@@ -138,6 +139,37 @@ int kara_oracle_compress_windows(const kara_oracle_layout* lay, uint16_t* k_pool
                                  int32_t* free_list, int32_t* free_count,
                                  const float* scores_in, float* scores_out,
                                  int32_t* idx_topk_out, int32_t* idx_final_out);
+
+/* Periodic compression policy (Alg. 1, reconstructed per reading G12; App. C.4; B.1, L275),
+ * the bookkeeping of ONE decoding step for a batch of running sequences, in Alg. 1's order:
+ *   l.2  every active sequence has generated one token: if its current length is a multiple of the block size the
+ *        token opens a new block, popped from the TOP of the free-list stack (sequences in batch order; reading G18);
+ *        seq_len += 1, uncompressed += 1.  A sequence that needs a block while the free list is empty is not advanced
+ *        and *exhausted is incremented (the serving engine would preempt it: out of scope).
+ *   l.3  g <- g + 1
+ *   l.4  if g > W and g mod delta == 0:
+ *   l.5    SELECT: sequences whose tail holds W uncompressed tokens in FULL blocks, the last (possibly partial) block
+ *          excluded (App. C.4): t = seq_len mod block_size, eligible iff uncompressed - t >= W; window start
+ *          h = seq_len - t - W.  The first max_select eligible sequences in batch order are taken (the paper takes "30
+ *          sequences", L275, and does not say which: reading G18).
+ *          For selected sequence number x: sel_ids[x] = s, sel_win_start[x] = h, sel_seq_lens[x] = seq_len,
+ *          sel_block_table[x][:] = block_table[s][:].  Rows x >= *sel_count get sel_ids = -1, sel_seq_lens = -1.
+ * `uncompressed` is the number of trailing tokens never compressed (buffer and partial block included); the paper's
+ * per-sequence variable "reset to 0 after each compression" (L354) counts the tokens beyond the compressed window, i.e.
+ * this counter minus the U + t tokens that kara_oracle_policy_commit leaves in it.  active may be NULL (all active). */
+int kara_oracle_policy_step(int n_seqs, int max_blocks, int block_size, int32_t* block_table, int32_t* seq_lens,
+                            int32_t* uncompressed, const uint8_t* active, int32_t* free_list, int32_t* free_count,
+                            int32_t* step_counter, int delta, int W, int max_select,
+                            int32_t* sel_ids, int32_t* sel_count, int32_t* sel_block_table, int32_t* sel_seq_lens,
+                            int32_t* sel_win_start, int32_t* exhausted);
+
+/* After the selected sub-batch has been compressed and committed (kara_oracle_compress_window on sel_block_table /
+ * sel_seq_lens / sel_win_start): UpdateMetadata of the running queue (Alg. 1 l.12): for x < sel_count, s = sel_ids[x]:
+ * block_table[s][:] = sel_block_table[x][:], seq_lens[s] = sel_seq_lens[x] (= h + keep + U + t), and the counter of
+ * uncompressed trailing tokens becomes U + t, t = new seq_len - (sel_win_start[x] + keep + U). */
+int kara_oracle_policy_commit(int max_blocks, const int32_t* sel_ids, int sel_count, const int32_t* sel_block_table,
+                              const int32_t* sel_seq_lens, const int32_t* sel_win_start, int keep, int U,
+                              int32_t* block_table, int32_t* seq_lens, int32_t* uncompressed);
 
 #ifdef __cplusplus
 }

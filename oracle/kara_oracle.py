@@ -80,6 +80,13 @@ def lib() -> C.CDLL:
             C.POINTER(Layout), u16p, u16p, C.c_int, C.c_int, C.c_int, i32p, C.c_int, i32p, i32p, C.c_int,
             u16p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int,
             i32p, i32p, f32p, f32p, i32p, i32p]
+        u8p = C.POINTER(C.c_uint8)
+        L.kara_oracle_policy_step.restype = C.c_int
+        L.kara_oracle_policy_step.argtypes = [C.c_int, C.c_int, C.c_int, i32p, i32p, i32p, u8p, i32p, i32p, i32p,
+                                              C.c_int, C.c_int, C.c_int, i32p, i32p, i32p, i32p, i32p, i32p]
+        L.kara_oracle_policy_commit.restype = C.c_int
+        L.kara_oracle_policy_commit.argtypes = [C.c_int, i32p, C.c_int, i32p, i32p, i32p, C.c_int, C.c_int,
+                                                i32p, i32p, i32p]
         _LIB = L
     return _LIB
 
@@ -220,3 +227,42 @@ def compress_window(layout: Layout, k_pool, v_pool, layer_begin, layer_end, bloc
         raise ValueError(f"kara_oracle_compress_window rc={rc}")
     out.update(scores=s_out, idx_topk=i_out, idx_final=f_out)
     return out
+
+
+def policy_step(block_table, seq_lens, uncompressed, active, free_list, free_count, step_counter, block_size,
+                delta, W, max_select):
+    """One decoding step of Alg. 1 (in place on the int32 arrays; step_counter / free_count are int32 [1]).
+    Returns dict(sel_ids, sel_count, sel_block_table, sel_seq_lens, sel_win_start, exhausted)."""
+    block_table = _chk(block_table, np.int32, "block_table")
+    n_seqs, max_blocks = block_table.shape
+    sel_ids = np.empty(max(max_select, 1), np.int32)
+    sel_sl = np.empty(max(max_select, 1), np.int32)
+    sel_ws = np.empty(max(max_select, 1), np.int32)
+    sel_bt = np.empty((max(max_select, 1), max_blocks), np.int32)
+    cnt = np.zeros(1, np.int32)
+    exh = np.zeros(1, np.int32)
+    act = None if active is None else _chk(active, np.uint8, "active")
+    rc = lib().kara_oracle_policy_step(
+        n_seqs, max_blocks, block_size, _p(block_table, C.c_int32), _p(_chk(seq_lens, np.int32, "seq_lens"), C.c_int32),
+        _p(_chk(uncompressed, np.int32, "uncompressed"), C.c_int32), _p(act, C.c_uint8),
+        _p(_chk(free_list, np.int32, "free_list"), C.c_int32), _p(_chk(free_count, np.int32, "free_count"), C.c_int32),
+        _p(_chk(step_counter, np.int32, "step_counter"), C.c_int32), delta, W, max_select,
+        _p(sel_ids, C.c_int32), _p(cnt, C.c_int32), _p(sel_bt, C.c_int32), _p(sel_sl, C.c_int32), _p(sel_ws, C.c_int32),
+        _p(exh, C.c_int32))
+    if rc:
+        raise ValueError(f"kara_oracle_policy_step rc={rc}")
+    return dict(sel_ids=sel_ids[:max_select], sel_count=int(cnt[0]), sel_block_table=sel_bt[:max_select],
+                sel_seq_lens=sel_sl[:max_select], sel_win_start=sel_ws[:max_select], exhausted=int(exh[0]))
+
+
+def policy_commit(sel, keep, U, block_table, seq_lens, uncompressed):
+    """UpdateMetadata of the running queue after the selected sub-batch was compressed (in place)."""
+    block_table = _chk(block_table, np.int32, "block_table")
+    rc = lib().kara_oracle_policy_commit(
+        block_table.shape[1], _p(np.ascontiguousarray(sel["sel_ids"], np.int32), C.c_int32), int(sel["sel_count"]),
+        _p(np.ascontiguousarray(sel["sel_block_table"], np.int32), C.c_int32),
+        _p(np.ascontiguousarray(sel["sel_seq_lens"], np.int32), C.c_int32),
+        _p(np.ascontiguousarray(sel["sel_win_start"], np.int32), C.c_int32), keep, U, _p(block_table, C.c_int32),
+        _p(_chk(seq_lens, np.int32, "seq_lens"), C.c_int32), _p(_chk(uncompressed, np.int32, "uncompressed"), C.c_int32))
+    if rc:
+        raise ValueError(f"kara_oracle_policy_commit rc={rc}")
