@@ -167,6 +167,38 @@ int kara_gather_debug(kara_cache* c, int what, int layer, int seq, int kv_head,
                       int max_blocks, void* out /*host*/, int64_t out_capacity_bytes,
                       int64_t* out_count /*host*/);
 
+/* Periodic compression policy on the device (Alg. 1, as reconstructed by DESIGN.md reading G12;
+ * App. C.4; B.1, L275): the bookkeeping of ONE decoding step of the running queue, asynchronous on `stream`.
+ *   l.2   every active sequence has generated one token (the caller's decode step writes its K/V row): a token at a block
+ *         boundary takes a block from the TOP of the attached free-list stack, sequences in batch order (reading G18);
+ *         seq_len += 1, uncompressed += 1.  A sequence that needs a block while the stack is empty (or its table row is
+ *         full) is not advanced and *exhausted is incremented — preemption is the serving engine's business.
+ *   l.3   *step_counter += 1  (= g)
+ *   l.4-5 if g > W and g mod delta == 0: SELECT the first max_select sequences, in batch order, whose tail holds W
+ *         uncompressed tokens in full blocks — t = seq_len mod block_size tokens of the partial last block are excluded
+ *         (App. C.4): eligible iff uncompressed - t >= W; window start h = seq_len - t - W.  Selected sequence number x
+ *         gets sel_ids[x] = s, sel_win_start[x] = h, sel_seq_lens[x] = seq_len, sel_block_table[x][:] = block_table[s][:];
+ *         rows x >= *sel_count get sel_ids = -1, sel_seq_lens = -1 ("absent": kara_compress_window skips them silently).
+ * The sel_* arrays ARE the sub-batch of the compression event: recompute the window queries of the selected sequences
+ * (sub-batch order), call kara_compress_window(n_seqs = max_select, sel_block_table, sel_seq_lens, sel_win_start, ...,
+ * KARA_COMMIT), then kara_policy_commit.  `uncompressed` [dev int32 n_seqs] counts the trailing tokens never compressed
+ * (buffer and partial block included: the paper's per-sequence variable, L354, counts the tokens beyond the last window,
+ * i.e. this minus U + t).  active [dev uint8 n_seqs] or NULL (all).  All sel_* are [dev], sized max_select
+ * (sel_block_table: max_select x max_blocks); step_counter, sel_count, exhausted are [dev int32 1]. */
+int kara_policy_step(kara_cache* c, int n_seqs, int32_t* block_table /*dev, in/out*/, int max_blocks,
+                     int32_t* seq_lens /*dev, in/out*/, int32_t* uncompressed /*dev, in/out*/,
+                     const uint8_t* active /*dev or NULL*/, int32_t* step_counter /*dev*/, int delta, int W,
+                     int max_select, int32_t* sel_ids, int32_t* sel_count, int32_t* sel_block_table,
+                     int32_t* sel_seq_lens, int32_t* sel_win_start, int32_t* exhausted, void* stream);
+
+/* Alg. 1 l.12 UpdateMetadata(e) for the running queue after the sub-batch was compressed and committed: for x < *sel_count,
+ * s = sel_ids[x]: block_table[s][:] = sel_block_table[x][:], seq_lens[s] = sel_seq_lens[x], and uncompressed[s] = U + t with
+ * t = sel_seq_lens[x] - (sel_win_start[x] + keep + U), keep = ceil(ratio (W-U)).  Asynchronous on `stream`. */
+int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, const int32_t* sel_count,
+                       const int32_t* sel_block_table, const int32_t* sel_seq_lens, const int32_t* sel_win_start,
+                       int W, int U, double ratio, int32_t* block_table /*dev*/, int max_blocks,
+                       int32_t* seq_lens /*dev*/, int32_t* uncompressed /*dev*/, void* stream);
+
 /* Synchronous: reads and clears the device status word (0 = no fault).  The word is sticky: it holds the
  * OR of the faults of every kara_compress_window call on this handle since the last kara_status(), as long
  * as those calls used the same workspace (the layer-range flow: several calls, KARA_COMMIT on the last). */

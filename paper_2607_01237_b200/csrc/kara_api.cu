@@ -434,6 +434,41 @@ int kara_gather_debug(kara_cache* c, int what, int layer, int seq, int kv_head, 
   }
 }
 
+int kara_policy_step(kara_cache* c, int n_seqs, int32_t* block_table, int max_blocks, int32_t* seq_lens,
+                     int32_t* uncompressed, const uint8_t* active, int32_t* step_counter, int delta, int W,
+                     int max_select, int32_t* sel_ids, int32_t* sel_count, int32_t* sel_block_table,
+                     int32_t* sel_seq_lens, int32_t* sel_win_start, int32_t* exhausted, void* stream) {
+  if (!c || !c->attached) return fail(KARA_EINVAL, "kara_policy_step: no pool attached");
+  if (n_seqs <= 0 || max_blocks <= 0 || delta <= 0 || W <= 0 || max_select <= 0)
+    return fail(KARA_EINVAL, "kara_policy_step: n_seqs=%d max_blocks=%d delta=%d W=%d max_select=%d", n_seqs, max_blocks,
+                delta, W, max_select);
+  if (!block_table || !seq_lens || !uncompressed || !step_counter || !sel_ids || !sel_count || !sel_block_table ||
+      !sel_seq_lens || !sel_win_start || !exhausted)
+    return fail(KARA_EINVAL, "kara_policy_step: null pointer argument");
+  KARA_CUDA(launch_policy_step(n_seqs, max_blocks, c->g.bs, c->g.bs_log2, delta, W, max_select, block_table, seq_lens,
+                               uncompressed, active, c->free_list, c->free_count, step_counter, sel_ids, sel_count,
+                               sel_block_table, sel_seq_lens, sel_win_start, exhausted,
+                               reinterpret_cast<cudaStream_t>(stream)));
+  return KARA_OK;
+}
+
+int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, const int32_t* sel_count,
+                       const int32_t* sel_block_table, const int32_t* sel_seq_lens, const int32_t* sel_win_start,
+                       int W, int U, double ratio, int32_t* block_table, int max_blocks, int32_t* seq_lens,
+                       int32_t* uncompressed, void* stream) {
+  if (!c) return fail(KARA_EINVAL, "null handle");
+  if (U < 0 || W <= U || max_select <= 0 || max_blocks <= 0) return fail(KARA_EINVAL, "kara_policy_commit: bad W/U/sizes");
+  const int keep = budget(W - U, ratio);
+  if (keep < 0) return fail(KARA_EINVAL, "ratio=%g outside (0,1]", ratio);
+  if (!sel_ids || !sel_count || !sel_block_table || !sel_seq_lens || !sel_win_start || !block_table || !seq_lens ||
+      !uncompressed)
+    return fail(KARA_EINVAL, "kara_policy_commit: null pointer argument");
+  KARA_CUDA(launch_policy_commit(max_select, max_blocks, keep, U, sel_ids, sel_count, sel_block_table, sel_seq_lens,
+                                 sel_win_start, block_table, seq_lens, uncompressed,
+                                 reinterpret_cast<cudaStream_t>(stream)));
+  return KARA_OK;
+}
+
 int kara_status(kara_cache* c, int32_t* status_out) {
   if (!c || !status_out) return fail(KARA_EINVAL, "null argument");
   *status_out = 0;

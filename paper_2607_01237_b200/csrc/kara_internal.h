@@ -96,6 +96,7 @@ __host__ __device__ inline int unit_count(const Call& c) { return c.n_layers * c
 // last window (window w covers [h + w W, h + (w+1) W)).  Returns false (and sets status bits) if the sequence must be skipped.
 __device__ inline bool window_of(const Call& c, int s, int& h, int& t, int& len) {
   len = c.seq_lens[s];
+  if (len < 0) { h = 0; t = 0; return false; }     // an absent row of a kara_policy_step sub-batch: skipped silently
   h = c.win_start ? c.win_start[s] : len - c.n_windows * c.W;
   t = len - h - c.n_windows * c.W;
   int bad = 0;
@@ -136,6 +137,15 @@ cudaError_t launch_score_simt(const Call& c, cudaStream_t st);
 cudaError_t launch_select_compact(const Call& c, cudaStream_t st);
 cudaError_t launch_compact_windows(const Call& c, cudaStream_t st);   // a4 of a multi-window call (n_windows > 1)
 cudaError_t launch_metadata(const Call& c, cudaStream_t st);
+cudaError_t launch_policy_step(int n_seqs, int max_blocks, int bs, int bs_log2, int delta, int W, int max_select,
+                               int32_t* block_table, int32_t* seq_lens, int32_t* uncompressed, const uint8_t* active,
+                               int32_t* free_list, int32_t* free_count, int32_t* step_counter, int32_t* sel_ids,
+                               int32_t* sel_count, int32_t* sel_block_table, int32_t* sel_seq_lens, int32_t* sel_win_start,
+                               int32_t* exhausted, cudaStream_t st);
+cudaError_t launch_policy_commit(int max_select, int max_blocks, int keep, int U, const int32_t* sel_ids,
+                                 const int32_t* sel_count, const int32_t* sel_block_table, const int32_t* sel_seq_lens,
+                                 const int32_t* sel_win_start, int32_t* block_table, int32_t* seq_lens,
+                                 int32_t* uncompressed, cudaStream_t st);
 cudaError_t launch_gather_rows(const Geom& g, const __nv_bfloat16* pool, int layer, int kv_head,
                                const int32_t* bt_row, int length, __nv_bfloat16* out, int32_t* status,
                                cudaStream_t st);

@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
       const int h = c.win_start ? c.win_start[s] : len - c.n_windows * c.W;
       const int t = len - h - c.n_windows * c.W;
       old_nb = (len + c.g.bs - 1) >> c.g.bs_log2;
-      ok = (h >= 0 && t >= 0 && old_nb <= c.max_blocks);
+      ok = (len >= 0 && h >= 0 && t >= 0 && old_nb <= c.max_blocks);   // len < 0: absent row of a policy sub-batch
       if (ok) {
         // the same validation select_compact ran: a sequence with a block id outside the pool in its window
         // was not compacted and is not committed (its table row, seq_len and the free list stay as they are)

@@ -125,7 +125,7 @@ __device__ __forceinline__ Seg decode_seg(const Call& c, long long g, long long 
   const int len = c.seq_lens[it.s];
   const int h0 = c.win_start ? c.win_start[it.s] : len - c.n_windows * c.W;   // first window of the sequence
   const int t = len - h0 - c.n_windows * c.W;
-  it.ok = (h0 >= 0 && t >= 0 && ((len + c.g.bs - 1) >> c.g.bs_log2) <= c.max_blocks);
+  it.ok = (len >= 0 && h0 >= 0 && t >= 0 && ((len + c.g.bs - 1) >> c.g.bs_log2) <= c.max_blocks);
   it.h = it.ok ? h0 + it.w * c.W : 0;
   it.fb = it.h >> c.g.bs_log2;
   it.off = it.h - (it.fb << c.g.bs_log2);

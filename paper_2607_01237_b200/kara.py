@@ -39,6 +39,8 @@ SYMBOLS = {
                                    _vp, _sz, _vp]),
     "kara_compress_window_host": (_i, [_vp, _i, _i, _i, _vp, _i, _vp, _vp, _vp, _i, _i, _i, _d, _i, _i,
                                        _u, _vp, _vp]),
+    "kara_policy_step": (_i, [_vp, _i, _vp, _i, _vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "kara_policy_commit": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp, _i, _i, _d, _vp, _i, _vp, _vp, _vp]),
     "kara_gather_debug": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i, _vp, _i64, C.POINTER(_i64)]),
     "kara_status": (_i, [_vp, C.POINTER(C.c_int32)]),
     "kara_last_launch_count": (_i, [_vp]),
@@ -187,6 +189,30 @@ class KaraCache:
                                                _ptr(seq_lens), _ptr(win_start), _ptr(window_q), Hq, W, U,
                                                float(ratio), alpha, gamma, flags, _ptr(fc), st))
         return int(fc[0])
+
+    # -- kara_policy_step / kara_policy_commit (Alg. 1 on the device) -----------------------------------------
+    def policy_step(self, block_table, seq_lens, uncompressed, active, step_counter, delta, W, sel, exhausted,
+                    stream: torch.cuda.Stream | None = None) -> None:
+        """`sel` = dict of device tensors ids [m], count [1], block_table [m, max_blocks], seq_lens [m], win_start [m]."""
+        n_seqs, max_blocks = block_table.shape
+        m = sel["ids"].numel()
+        assert sel["block_table"].shape == (m, max_blocks) and sel["block_table"].is_contiguous()
+        for x in (block_table, seq_lens, uncompressed, step_counter, exhausted, *sel.values()):
+            assert x.is_cuda and x.dtype == torch.int32 and x.is_contiguous()
+        assert active is None or (active.is_cuda and active.dtype == torch.uint8)
+        st = (stream or torch.cuda.current_stream(block_table.device)).cuda_stream
+        _check(lib().kara_policy_step(self._h, n_seqs, _ptr(block_table), max_blocks, _ptr(seq_lens), _ptr(uncompressed),
+                                      _ptr(active), _ptr(step_counter), delta, W, m, _ptr(sel["ids"]), _ptr(sel["count"]),
+                                      _ptr(sel["block_table"]), _ptr(sel["seq_lens"]), _ptr(sel["win_start"]),
+                                      _ptr(exhausted), st))
+
+    def policy_commit(self, sel, W, U, ratio, block_table, seq_lens, uncompressed,
+                      stream: torch.cuda.Stream | None = None) -> None:
+        m = sel["ids"].numel()
+        st = (stream or torch.cuda.current_stream(block_table.device)).cuda_stream
+        _check(lib().kara_policy_commit(self._h, m, _ptr(sel["ids"]), _ptr(sel["count"]), _ptr(sel["block_table"]),
+                                        _ptr(sel["seq_lens"]), _ptr(sel["win_start"]), W, U, float(ratio),
+                                        _ptr(block_table), block_table.shape[1], _ptr(seq_lens), _ptr(uncompressed), st))
 
     # -- kara_gather_debug -----------------------------------------------------------------------------
     def gather_debug(self, what: int, layer: int, seq: int, kv_head: int, block_table: torch.Tensor | None = None,
