@@ -27,6 +27,12 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
+#ifndef KARA_SEL_VEC
+#define KARA_SEL_VEC 4      // 16-byte vectors per thread and tensor in one compaction pass (measured: 4 x 5 CTAs/SM beats 8 x 3 at cfg4)
+#endif
+#ifndef KARA_SEL_OCC
+#define KARA_SEL_OCC 5
+#endif
 
 struct Scratch {
   int hist[256];
@@ -163,7 +169,7 @@ __device__ __forceinline__ void compact_rows_inplace(const Call& c, int layer, i
                                                      long long* s_off, int stage_rows) {
   const int tid = threadIdx.x;
   const int vpr = c.g.d / 8;                                   // 16-byte vectors per row
-  constexpr int kVecPerThread = 8;                             // per tensor
+  constexpr int kVecPerThread = KARA_SEL_VEC;                  // per tensor
   const int rows_per_pass = kThreads * kVecPerThread / vpr;    // 128 rows at d = 128, 256 at d = 64
   __nv_bfloat16* kp = const_cast<__nv_bfloat16*>(c.k_pool);
   __nv_bfloat16* vp = const_cast<__nv_bfloat16*>(c.v_pool);
@@ -197,7 +203,7 @@ __device__ __forceinline__ void compact_rows_inplace(const Call& c, int layer, i
   }
 }
 
-__global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call c, int stage_rows, int off_bytes) {
+__global__ void __launch_bounds__(kThreads, KARA_SEL_OCC) select_compact_kernel(const Call c, int stage_rows, int off_bytes) {
   // programmatic dependent launch: this grid may be scheduled while the score kernel drains; nothing the
   // score kernel writes is read before the wait, and the metadata kernel behind may be scheduled early too
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -315,7 +321,7 @@ __global__ void __launch_bounds__(kThreads, 3) select_compact_kernel(const Call 
 //   new[h + w (keep+U) + keep + c] = old[h + w W + n + c]        c < U
 //   new[h + NW (keep+U) + c]       = old[h + NW W + c]           c < t
 // F_w is read from the workspace (written by select_compact_kernel of the same call).
-__global__ void __launch_bounds__(kThreads, 3) compact_windows_kernel(const Call c, int stage_rows) {
+__global__ void __launch_bounds__(kThreads, KARA_SEL_OCC) compact_windows_kernel(const Call c, int stage_rows) {
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   extern __shared__ __align__(16) unsigned char smem_raw[];
