@@ -493,3 +493,45 @@ int kara_oracle_policy_commit(int max_blocks, const int32_t* sel_ids, int sel_co
   }
   return KARA_ORACLE_OK;
 }
+
+/* ---------------------------------------------------------------------------------------- */
+/* App. C.2 query projection + rotary embedding (reading G19). */
+static uint16_t double_to_bf16_rne(double x) {
+  float f = (float)x;                       /* double -> float is exact enough: a bf16 keeps 8 of the float's 24 bits */
+  uint32_t u;
+  memcpy(&u, &f, sizeof u);
+  if ((u & 0x7f800000u) == 0x7f800000u) return (uint16_t)(u >> 16);       /* inf / nan */
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+int kara_oracle_window_queries(const uint16_t* hidden, const uint16_t* wq, const int32_t* positions, double rope_theta,
+                               int T, int d_model, int n_q_heads, int d, uint16_t* out) {
+  if (!hidden || !wq || !out || T < 0 || d_model <= 0 || n_q_heads <= 0 || d <= 0 || (d & 1)) return KARA_ORACLE_EINVAL;
+  double* q = (double*)malloc(sizeof(double) * (size_t)d);
+  if (!q) return KARA_ORACLE_EINVAL;
+  for (int t = 0; t < T; ++t) {
+    for (int h = 0; h < n_q_heads; ++h) {
+      for (int c = 0; c < d; ++c) {
+        const uint16_t* wrow = wq + ((long)h * d + c) * d_model;
+        double acc = 0.0;
+        for (int k = 0; k < d_model; ++k)
+          acc += kara_oracle_bf16_to_double(hidden[(long)t * d_model + k]) * kara_oracle_bf16_to_double(wrow[k]);
+        q[c] = acc;
+      }
+      uint16_t* o = out + ((long)t * n_q_heads + h) * d;
+      if (!positions) {
+        for (int c = 0; c < d; ++c) o[c] = double_to_bf16_rne(q[c]);
+      } else {
+        for (int c = 0; c < d / 2; ++c) {
+          const double a = (double)positions[t] * pow(rope_theta, -2.0 * (double)c / (double)d);
+          const double cs = cos(a), sn = sin(a);
+          o[c] = double_to_bf16_rne(q[c] * cs - q[c + d / 2] * sn);
+          o[c + d / 2] = double_to_bf16_rne(q[c + d / 2] * cs + q[c] * sn);
+        }
+      }
+    }
+  }
+  free(q);
+  return KARA_ORACLE_OK;
+}

@@ -171,6 +171,17 @@ int kara_oracle_policy_commit(int max_blocks, const int32_t* sel_ids, int sel_co
                               const int32_t* sel_seq_lens, const int32_t* sel_win_start, int keep, int U,
                               int32_t* block_table, int32_t* seq_lens, int32_t* uncompressed);
 
+/* Window-query producer (App. C.2: at each compression "we run an additional forward pass on the tokens
+ * in the current window ... we compute only the query projections, ..."): the query states of T window tokens
+ * of one layer from their (normalised) hidden states,
+ *     q[t][h][:] = RoPE_{pos[t]}( sum_k hidden[t][k] * wq[h d + :][k] )
+ * bf16 inputs widened, products and sums in double, rounded ONCE to bf16 (round to nearest even).  Reading G19:
+ * rotary embedding in the rotate-half pairing of the paper's models (Llama / Qwen): for c < d/2, f_c = theta^(-2c/d),
+ * a = pos f_c:  out[c] = q[c] cos a - q[c+d/2] sin a,  out[c+d/2] = q[c+d/2] cos a + q[c] sin a;  no bias, no q-norm.
+ * positions == NULL: no rotary embedding.  hidden [T][d_model], wq [n_q_heads*d][d_model], out [T][n_q_heads][d] (bf16 bits). */
+int kara_oracle_window_queries(const uint16_t* hidden, const uint16_t* wq, const int32_t* positions, double rope_theta,
+                               int T, int d_model, int n_q_heads, int d, uint16_t* out);
+
 #ifdef __cplusplus
 }
 #endif

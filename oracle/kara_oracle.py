@@ -87,6 +87,8 @@ def lib() -> C.CDLL:
         L.kara_oracle_policy_commit.restype = C.c_int
         L.kara_oracle_policy_commit.argtypes = [C.c_int, i32p, C.c_int, i32p, i32p, i32p, C.c_int, C.c_int,
                                                 i32p, i32p, i32p]
+        L.kara_oracle_window_queries.restype = C.c_int
+        L.kara_oracle_window_queries.argtypes = [u16p, u16p, i32p, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, u16p]
         _LIB = L
     return _LIB
 
@@ -266,3 +268,18 @@ def policy_commit(sel, keep, U, block_table, seq_lens, uncompressed):
         _p(_chk(seq_lens, np.int32, "seq_lens"), C.c_int32), _p(_chk(uncompressed, np.int32, "uncompressed"), C.c_int32))
     if rc:
         raise ValueError(f"kara_oracle_policy_commit rc={rc}")
+
+
+def window_queries(hidden_bits, wq_bits, positions, rope_theta, n_q_heads, d):
+    """hidden uint16 [T, Dm], wq uint16 [Hq*d, Dm] (bf16 bits), positions int32 [T] or None -> uint16 [T, Hq, d]."""
+    hidden_bits = _chk(hidden_bits, np.uint16, "hidden")
+    wq_bits = _chk(wq_bits, np.uint16, "wq")
+    T, Dm = hidden_bits.shape
+    assert wq_bits.shape == (n_q_heads * d, Dm)
+    pos = None if positions is None else _chk(np.ascontiguousarray(positions, np.int32), np.int32, "positions")
+    out = np.empty((T, n_q_heads, d), np.uint16)
+    rc = lib().kara_oracle_window_queries(_p(hidden_bits, C.c_uint16), _p(wq_bits, C.c_uint16), _p(pos, C.c_int32),
+                                          float(rope_theta), T, Dm, n_q_heads, d, _p(out, C.c_uint16))
+    if rc:
+        raise ValueError(f"kara_oracle_window_queries rc={rc}")
+    return out
