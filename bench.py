@@ -367,6 +367,33 @@ def derived(res, peaks, world=1, total_ms=None, steps=1):
                 t_tensor_ms=t_tensor_ms, t_hbm_ms=t_hbm_ms, step_frac=max(t_tensor_ms, t_hbm_ms) / ms_per_step)
 
 
+def measure_producer(dev, peaks, T=64 * 512, Dm=5120, Hq=40, d=128, steps=10):
+    """kara_window_queries (Q projection + RoPE into the window_q layout) for one layer of 64 windows of 512
+    tokens at the Qwen3-14B shape; a GEMM, so its roofline is the bf16 tensor peak."""
+    import torch
+    from paper_2607_01237_b200 import kara
+    hid = torch.randn(T, Dm, device=dev).to(torch.bfloat16)
+    wq = (torch.randn(Hq * d, Dm, device=dev) / Dm ** 0.5).to(torch.bfloat16)
+    pos = (torch.arange(T, device=dev, dtype=torch.int32) % 512) + 20000
+    out = torch.empty(T, Hq, d, dtype=torch.bfloat16, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ms = []
+    for it in range(3 + steps):
+        flush.zero_()
+        ev0.record()
+        kara.kara_window_queries(hid, wq, pos, 1e6, Hq, d, out=out, max_position=32768)
+        ev1.record()
+        torch.cuda.synchronize()
+        if it >= 3:
+            ms.append(ev0.elapsed_time(ev1))
+    t = sum(ms) / len(ms)
+    tf = 2.0 * T * Dm * Hq * d / (t * 1e-3) / 1e12
+    return {"workload": f"SURVEY 8(f)-4 window-query producer: {T} tokens x d_model {Dm} -> {Hq} heads x {d}, RoPE fused",
+            "steps": steps, "ms_per_step": t, "tflops": tf, "roofline_frac": tf / peaks["bf16_tflops"], "bound": "tensor",
+            "window_queries_per_s": T / (t * 1e-3)}
+
+
 # -------------------------------------------------------------------------------------------------
 def run_gpu(args):
     import torch
@@ -439,6 +466,7 @@ def run_gpu(args):
                          "roofline_frac": dd["score_tflops"] / peaks["bf16_tflops"], "score_kernel_ms": dd["score_ms"],
                          "step_roofline_frac": dd["step_frac"], "freed_blocks_per_step": r["freed"],
                          "gpu_launches": r["launches"], "sm_mhz": r["clocks"]["sm_mhz"]}
+        per["window_q_producer"] = measure_producer(dev, peaks)
         line["per_config"] = per
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:

@@ -199,6 +199,24 @@ int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, co
                        int W, int U, double ratio, int32_t* block_table /*dev*/, int max_blocks,
                        int32_t* seq_lens /*dev*/, int32_t* uncompressed /*dev*/, void* stream);
 
+/* Window-query producer (App. C.2: at each compression the window's query states are recomputed — "we compute
+ * only the query projections, the causal attention against the cached prefix KV states, and the FFN").  This is
+ * the projection step for ONE layer, written directly in the layout kara_compress_window reads:
+ *     window_q_out[t][h][:] = RoPE_{positions[t]}( hidden[t][:] . wq[h*head_dim + :][:]^T )      bf16 in / out, fp32 accumulate
+ * Reading G19: rotary embedding in the rotate-half pairing of the paper's models — for c < d/2, f_c = theta^(-2c/d),
+ * a = pos f_c: out[c] = q[c] cos a - q[c+d/2] sin a, out[c+d/2] = q[c+d/2] cos a + q[c] sin a — no bias, no q-norm; the hidden
+ * states (the layer's normalised inputs, i.e. everything before the projection) are the caller's.
+ *   hidden        [dev bf16 n_tokens x d_model]   d_model a multiple of 64; 16-byte aligned
+ *   wq            [dev bf16 (n_q_heads*head_dim) x d_model]
+ *   positions     [dev int32 n_tokens] in [0, max_position], or NULL: no rotary embedding
+ *   window_q_out  [dev bf16 n_tokens x n_q_heads x head_dim]  (tokens in the order of the call's window_q: sequence, token)
+ *   workspace     [dev] >= kara_window_queries_workspace_bytes(max_position, head_dim) (cos / sin tables; unused without positions)
+ * Asynchronous on `stream`.  One hand-written tcgen05 / TMA GEMM with the rotary embedding fused into its epilogue. */
+size_t kara_window_queries_workspace_bytes(int max_position, int head_dim);
+int kara_window_queries(const void* hidden /*dev*/, const void* wq /*dev*/, const int32_t* positions /*dev or NULL*/,
+                        int max_position, double rope_theta, int n_tokens, int d_model, int n_q_heads, int head_dim,
+                        void* window_q_out /*dev*/, void* workspace /*dev*/, size_t workspace_bytes, void* stream);
+
 /* Synchronous: reads and clears the device status word (0 = no fault).  The word is sticky: it holds the
  * OR of the faults of every kara_compress_window call on this handle since the last kara_status(), as long
  * as those calls used the same workspace (the layer-range flow: several calls, KARA_COMMIT on the last). */

@@ -469,6 +469,28 @@ int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, co
   return KARA_OK;
 }
 
+size_t kara_window_queries_workspace_bytes(int max_position, int head_dim) {
+  if (head_dim != 64 && head_dim != 128) return 0;
+  return qproj_workspace_bytes(max_position, head_dim);
+}
+
+int kara_window_queries(const void* hidden, const void* wq, const int32_t* positions, int max_position, double rope_theta,
+                        int n_tokens, int d_model, int n_q_heads, int head_dim, void* window_q_out, void* workspace,
+                        size_t workspace_bytes, void* stream) {
+  if (!hidden || !wq || !window_q_out || n_tokens < 0 || n_q_heads <= 0)
+    return fail(KARA_EINVAL, "kara_window_queries: null pointer or bad sizes");
+  if (head_dim != 64 && head_dim != 128) return fail(KARA_EUNSUPPORTED, "head_dim=%d: need 64 or 128", head_dim);
+  if (d_model <= 0 || d_model % 64 != 0) return fail(KARA_EUNSUPPORTED, "d_model=%d: need a positive multiple of 64", d_model);
+  if (((uintptr_t)hidden | (uintptr_t)wq | (uintptr_t)window_q_out) & 15u)
+    return fail(KARA_EINVAL, "kara_window_queries: hidden, wq and window_q_out must be 16-byte aligned");
+  if (positions && (!workspace || max_position < 0 || !(rope_theta > 1.0)))
+    return fail(KARA_EINVAL, "kara_window_queries: rotary embedding needs a workspace, max_position >= 0 and theta > 1");
+  const int rc = qproj_launch(hidden, wq, positions, max_position, rope_theta, n_tokens, d_model, n_q_heads, head_dim,
+                              window_q_out, workspace, workspace_bytes, reinterpret_cast<cudaStream_t>(stream));
+  if (rc != KARA_OK) return fail(rc, "kara_window_queries: %s", qproj_error());
+  return KARA_OK;
+}
+
 int kara_status(kara_cache* c, int32_t* status_out) {
   if (!c || !status_out) return fail(KARA_EINVAL, "null argument");
   *status_out = 0;

@@ -146,6 +146,11 @@ cudaError_t launch_policy_commit(int max_select, int max_blocks, int keep, int U
                                  const int32_t* sel_count, const int32_t* sel_block_table, const int32_t* sel_seq_lens,
                                  const int32_t* sel_win_start, int32_t* block_table, int32_t* seq_lens,
                                  int32_t* uncompressed, cudaStream_t st);
+// window-query producer (qproj.cu): returns KARA_OK / KARA_E*; qproj_error() has the message
+size_t qproj_workspace_bytes(int max_position, int d);
+int qproj_launch(const void* hidden, const void* wq, const int32_t* positions, int max_position, double theta, int T,
+                 int Dm, int Hq, int d, void* out, void* workspace, size_t workspace_bytes, cudaStream_t st);
+const char* qproj_error();
 cudaError_t launch_gather_rows(const Geom& g, const __nv_bfloat16* pool, int layer, int kv_head,
                                const int32_t* bt_row, int length, __nv_bfloat16* out, int32_t* status,
                                cudaStream_t st);

@@ -41,6 +41,8 @@ SYMBOLS = {
                                        _u, _vp, _vp]),
     "kara_policy_step": (_i, [_vp, _i, _vp, _i, _vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "kara_policy_commit": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp, _i, _i, _d, _vp, _i, _vp, _vp, _vp]),
+    "kara_window_queries_workspace_bytes": (_sz, [_i, _i]),
+    "kara_window_queries": (_i, [_vp, _vp, _vp, _i, _d, _i, _i, _i, _i, _vp, _vp, _sz, _vp]),
     "kara_gather_debug": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i, _vp, _i64, C.POINTER(_i64)]),
     "kara_status": (_i, [_vp, C.POINTER(C.c_int32)]),
     "kara_last_launch_count": (_i, [_vp]),
@@ -83,6 +85,29 @@ def _ptr(t: torch.Tensor | None) -> int | None:
 
 def kara_budget(n: int, ratio: float) -> int:
     return int(lib().kara_budget(int(n), float(ratio)))
+
+
+def kara_window_queries(hidden: torch.Tensor, wq: torch.Tensor, positions: torch.Tensor | None, rope_theta: float,
+                        n_q_heads: int, head_dim: int, out: torch.Tensor | None = None, max_position: int | None = None,
+                        stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+    """kara_window_queries: hidden [T, Dm] bf16, wq [Hq*d, Dm] bf16, positions int32 [T] or None -> [T, Hq, d] bf16."""
+    T, Dm = hidden.shape
+    assert hidden.is_cuda and hidden.is_contiguous() and hidden.dtype == torch.bfloat16
+    assert wq.shape == (n_q_heads * head_dim, Dm) and wq.is_contiguous() and wq.dtype == torch.bfloat16
+    if out is None:
+        out = torch.empty(T, n_q_heads, head_dim, dtype=torch.bfloat16, device=hidden.device)
+    assert out.is_contiguous() and out.dtype == torch.bfloat16 and out.numel() == T * n_q_heads * head_dim
+    ws = None
+    if positions is not None:
+        assert positions.dtype == torch.int32 and positions.is_cuda and positions.numel() == T
+        if max_position is None:
+            max_position = int(positions.max()) if T else 0
+        ws = torch.empty(max(int(lib().kara_window_queries_workspace_bytes(max_position, head_dim)), 16), dtype=torch.uint8,
+                         device=hidden.device)
+    st = (stream or torch.cuda.current_stream(hidden.device)).cuda_stream
+    _check(lib().kara_window_queries(_ptr(hidden), _ptr(wq), _ptr(positions), max_position or 0, float(rope_theta), T, Dm,
+                                     n_q_heads, head_dim, _ptr(out), _ptr(ws), ws.numel() if ws is not None else 0, st))
+    return out
 
 
 class KaraCache:
