@@ -305,7 +305,8 @@ def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False,
     if score_path != 2 and not simt:
         # north_star: no multi-backend dispatch — a bench number from the CUDA-core kernel is not a bench number
         raise SystemExit(f"bench.py: workload {name} did not run on the tcgen05/TMA score kernel "
-                         f"(kara_last_score_path = {score_path}); pass --simt to time the CUDA-core kernel on purpose")
+                         f"(kara_last_score_path = {score_path}: {cache.last_score_path_reason()}); pass --simt to time the "
+                         "CUDA-core kernel on purpose")
 
     step_ms, score_ms = [], []
     if dist:

@@ -227,6 +227,9 @@ int kara_last_launch_count(const kara_cache* c);
 
 /* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA. */
 int kara_last_score_path(const kara_cache* c);
+/* "" if the tcgen05 kernel ran, else why the CUDA-core kernel did (KARA_SCORE_SIMT, or a shape / device the tcgen05
+ * kernel does not take).  The CUDA-core kernel is a cross-check, not a second backend: bench.py refuses its numbers. */
+const char* kara_last_score_path_reason(const kara_cache* c);
 
 /* Device time of the score kernel (a1) alone: when enabled, every kara_compress_window call
  * brackets its score launch with CUDA events on `stream`; kara_score_kernel_ms() synchronises on

@@ -24,6 +24,7 @@ struct kara_cache {
   Call last{};
   int last_launches = 0;
   int last_score_path = 0;
+  const char* last_score_reason = "";   // why the CUDA-core kernel ran ("" when the tcgen05 kernel did)
   // sticky device status word: not cleared between the calls of a step (see kara_status)
   const void* status_ws = nullptr;
   bool status_pending = false;
@@ -275,6 +276,7 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
     rc = score_tc_launch(&c->tc, k, st, &nl);    // sets k.part_T / part_nc / part_tpu
     if (rc != KARA_OK) return fail(rc, "score_tc_launch: %s", score_tc_error());
     c->last_score_path = 2;
+    c->last_score_reason = "";
     launches += nl;
   } else {
     const int rows = (W - k.q_row_begin) * k.G;
@@ -284,6 +286,8 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
     KARA_CUDA(launch_score_simt(k, st));
     ++launches;
     c->last_score_path = 1;
+    // never silent: the reason is kept for kara_last_score_path_reason (bench.py refuses to report such a run)
+    c->last_score_reason = (flags & KARA_SCORE_SIMT) ? "KARA_SCORE_SIMT was set" : score_tc_unsupported_reason(c->tc, k);
   }
   if (c->timing) { KARA_CUDA(cudaEventRecord(c->ev1, st)); c->ev_recorded = true; }
 
@@ -504,6 +508,7 @@ int kara_status(kara_cache* c, int32_t* status_out) {
 
 int kara_last_launch_count(const kara_cache* c) { return c ? c->last_launches : 0; }
 int kara_last_score_path(const kara_cache* c) { return c ? c->last_score_path : 0; }
+const char* kara_last_score_path_reason(const kara_cache* c) { return c && c->last_score_reason ? c->last_score_reason : ""; }
 
 int kara_enable_score_timing(kara_cache* c, int enable) {
   if (!c) return fail(KARA_EINVAL, "null handle");

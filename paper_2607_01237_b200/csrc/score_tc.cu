@@ -55,19 +55,6 @@ constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works 
 constexpr int kRegsB = 80, kRegsC = 120, kRegsOther = 40;
 thread_local char g_tc_err[256] = "";
 
-#ifndef KARA_B_PREFETCH
-#define KARA_B_PREFETCH 0                      // 1: the TMEM load of a tile's second piece is issued before the exponentials of the first
-#endif
-#ifndef KARA_B_SHAPE
-#define KARA_B_SHAPE 0                         // TMEM shape of pass B: 0 = 32x32b (thread = lane), 1 = 16x32bx2 (16 lanes x two 32-column pieces)
-#endif
-#if KARA_B_SHAPE == 0
-#define KARA_B_LD tmem_ld_32x32b_x32
-#define KARA_B_ST tmem_st_32x32b_x32
-#else
-#define KARA_B_LD tmem_ld_16x32bx2_x32
-#define KARA_B_ST tmem_st_16x32bx2_x32
-#endif
 #ifdef KARA_TC_TRACE
 // debug build: clock64() stamps of CTA 0's warp roles per tile (see kara_tc_trace_read below)
 constexpr int kTraceTiles = 64, kTraceEv = 8, kTraceRoles = 5;   // roles: 0 = B warp 0, 1 = B warp 15, 2 = MMA, 3 = C warp 16, 4 = C warp 17
@@ -171,15 +158,10 @@ __device__ __forceinline__ void pass_b_body(uint32_t (&r)[32], int& z_out, float
   uint64_t la = pk2(0.f, 0.f), lb = pk2(0.f, 0.f);
 #pragma unroll
   for (int i = 0; i < 16; ++i) {
-    // kPolyMask: column pairs whose exponentials run on the FMA pipe (never on a ragged piece, where masked
-    // columns must come out as exact zeros)
-    const bool poly = !RAGGED && ((kPolyMask >> (i & 7)) & 1);
     float a, b;
-    if (poly) exp2_poly2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b);
-#ifdef KARA_DBG_NO_EX2
-    else { upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b); }
-#else
-    else { upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b); a = ex2(a); b = ex2(b); }
+    upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b);
+#ifndef KARA_DBG_NO_EX2                        // (diagnostic build: what the kernel costs without a single exponential)
+    a = ex2(a); b = ex2(b);
 #endif
     if (i & 1) lb = add2(lb, pk2(a, b)); else la = add2(la, pk2(a, b));
     r[2 * i] = __float_as_uint(a); r[2 * i + 1] = __float_as_uint(b);
@@ -550,18 +532,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
     // All 16 warps sweep half 0, then half 1, so the refill of a half has a whole half-sweep of slack and four warps per
     // scheduler feed the MUFU pipe at any time.
     const int q = warp & 3, cq = warp >> 2;
-#if KARA_B_SHAPE == 0
     // 32x32b: warp (q, cq) holds rows [32 q, + 32) x piece column cq; thread = TMEM lane
     const int pcq = cq, colw0 = cq * 32, colw_n = 32;
     const int row = q * 32 + lane;
     const uint32_t tq = tmem_base + ((uint32_t)(q * 32) << 16) + cq * 32;
-#else
-    // 16x32bx2: warp (q, cq) holds rows [32 q + 16 (cq & 1), + 16) x the 64 columns [64 (cq >> 1), + 64): thread t has row
-    // 32 q + 16 (cq & 1) + (t & 15), piece column 2 (cq >> 1) + (t >> 4)
-    const int pcq = 2 * (cq >> 1) + (lane >> 4), colw0 = (cq >> 1) * 64, colw_n = 64;
-    const int row = q * 32 + 16 * (cq & 1) + (lane & 15);
-    const uint32_t tq = tmem_base + ((uint32_t)(q * 32 + 16 * (cq & 1)) << 16) + (cq >> 1) * 64;
-#endif
     const float cs = kLog2e * rsqrtf((float)D);
     int tile_iter = 0;
     for (long long g = g_begin; g < g_end;) {
@@ -581,34 +555,25 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 0);
         mbar_wait(tfull + 8 * (b * 2 + 0), par);
         tc_fence_after();
-        KARA_B_LD(ta, ra);                      // (an inactive piece is loaded too and ignored)
+        tmem_ld_32x32b_x32(ta, ra);                      // (an inactive piece is loaded too and ignored)
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 1);
         // the TMEM load of piece 1 runs under the exponentials of piece 0 (in the B-bound steady state its S half
         // has landed long before; a starved B warp loses at most the time between the two MMA halves here)
-#if KARA_B_PREFETCH
-        mbar_wait(tfull + 8 * (b * 2 + 1), par);
-        tc_fence_after();
         tmem_wait_ld();
-        KARA_B_LD(ta + kHalf, rb);
-#else
-        tmem_wait_ld();
-#endif
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 2);
         // ---- pass B: e = 2^(s c - z) in place; (z, l) of (row, piece); the thread owns row 32 q + lane ----
         if (act0) {
           pass_b_piece(ra, z0, l0, cs, colw0, colw_n, pcq * 32, c_lo, c_hi);
-          KARA_B_ST(ta, ra);
+          tmem_st_32x32b_x32(ta, ra);
         }
-#if !KARA_B_PREFETCH
         mbar_wait(tfull + 8 * (b * 2 + 1), par);
         tc_fence_after();
-        KARA_B_LD(ta + kHalf, rb);
-#endif
+        tmem_ld_32x32b_x32(ta + kHalf, rb);
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 3);
         tmem_wait_ld();
         if (act1) {
           pass_b_piece(rb, z1, l1, cs, kHalf + colw0, colw_n, kHalf + pcq * 32, c_lo, c_hi);
-          KARA_B_ST(ta + kHalf, rb);
+          tmem_st_32x32b_x32(ta + kHalf, rb);
         }
         rstat[(b * 4 + pcq) * 128 + row] = make_uint4((uint32_t)z0, __float_as_uint(l0), (uint32_t)z1, __float_as_uint(l1));
         if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 4);
@@ -744,15 +709,16 @@ int score_tc_attach(ScoreTcState* s, const Geom& g, void* k_pool) {
   return KARA_OK;
 }
 
-bool score_tc_supported(const ScoreTcState& s, const Call& c) {
-  if (!s.ready) return false;
-  if (c.g.d != 64 && c.g.d != 128) return false;
-  if (c.g.bs > kKeysPerCta) return false;
-  if (cluster_size_for(c) == 0) return false;
+const char* score_tc_unsupported_reason(const ScoreTcState& s, const Call& c) {
+  if (!s.ready) return "no sm_100 device, or the K pool has 2^31 rows or more (beyond one tensor map's coordinates)";
+  if (c.g.d != 64 && c.g.d != 128) return "head_dim not 64 or 128";
+  if (c.g.bs > kKeysPerCta) return "block_size above 256";
+  if (cluster_size_for(c) == 0) return "window needs more than 8 CTAs of 256 keys";
   const unsigned long long toks = (unsigned long long)c.n_layers * c.n_seqs * c.n_windows * c.W;
-  if (toks >= (1ull << 31)) return false;
-  return true;
+  if (toks >= (1ull << 31)) return "2^31 window tokens or more in one call";
+  return nullptr;
 }
+bool score_tc_supported(const ScoreTcState& s, const Call& c) { return score_tc_unsupported_reason(s, c) == nullptr; }
 
 int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) {
   // window_q tensor map: [d][n_q_heads][layers*seqs*W tokens], box 64 x 1 x 128, 128B swizzle

@@ -17,6 +17,8 @@ struct ScoreTcState {
 int score_tc_attach(ScoreTcState* s, const Geom& g, void* k_pool);
 // True if the tcgen05 kernel takes this call's shapes (else the SIMT kernel runs).
 bool score_tc_supported(const ScoreTcState& s, const Call& c);
+// nullptr if the tcgen05 kernel takes the call, else why not (kara_last_score_path_reason)
+const char* score_tc_unsupported_reason(const ScoreTcState& s, const Call& c);
 // Launches the kernel(s); sets c.parts to the number of partial column-sum strips it writes.
 int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches);
 const char* score_tc_error();

@@ -1,6 +1,6 @@
 // score_tc_ptx.cuh — building blocks of the tcgen05 score kernel (score_tc.cu): tile constants, the
 // integer-shift conventions of the online softmax, and thin wrappers around the sm_100a PTX they use (mbarrier,
-// TMA, tcgen05 alloc / mma / commit / ld / st, cluster addressing, packed f32x2 arithmetic, the FMA-pipe exp2).
+// TMA, tcgen05 alloc / mma / commit / ld / st, cluster addressing, packed f32x2 arithmetic).
 // Everything is in an anonymous namespace: each translation unit gets its own copy.
 #pragma once
 #include <cuda.h>
@@ -25,10 +25,6 @@ constexpr int kMagicBits = 0x4B400000;
 // are clamped to z <= kZLim (|logit| log2e / sqrt(d) beyond that is not served) and floored at
 // -kZLim, which is also the shift of a piece with no valid key (its l is 0)
 constexpr float kZLim = 32000.f;
-#ifndef KARA_POLY_MASK
-#define KARA_POLY_MASK 0x00                   // bit i: column group i of 8 uses the FMA-pipe polynomial (measured: 0x52 is 7 % slower)
-#endif
-constexpr unsigned kPolyMask = KARA_POLY_MASK;
 constexpr int kZFloor = kMagicBits - 32000;
 
 // ------------------------------------------------------------------------------------------------
@@ -222,24 +218,6 @@ __device__ __forceinline__ void tmem_st_32x32b_x32(uint32_t taddr, const uint32_
       "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
       :: KARA_TMEM_IN32(r), "r"(taddr) : "memory");
 }
-// 16 lanes x (32 + 32) columns: thread t < 16 gets lane t, columns [c, c+32); thread t >= 16 gets lane t-16, columns
-// [c+32, c+64) — one S row piece of 32 consecutive columns per thread.  (The 32x32b shape, one lane per thread, would
-// give a thread its row directly, but measured on B200 it reads TMEM at 57 B/clk per SM however many warps issue it;
-// the 16-lane shapes reach 200+ B/clk: _work microbenchmark.)
-__device__ __forceinline__ void tmem_ld_16x32bx2_x32(uint32_t taddr, uint32_t (&r)[32]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.16x32bx2.x32.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32], 32;"
-      : KARA_TMEM_REGS32(r) : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_st_16x32bx2_x32(uint32_t taddr, const uint32_t (&r)[32]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.16x32bx2.x32.b32 [%32], 32, "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
-      :: KARA_TMEM_IN32(r), "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -276,28 +254,6 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
   uint64_t r;
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
   return r;
-}
-// 2^x for a pair of x <= 0.5 on the FMA pipe (the MUFU pipe, 16 ex2/clk/SM, is the scarcer resource
-// of pass B: one ex2 per 2 d tensor FLOPs): x = n + f, n = round(x) by the magic-number add, f in
-// [-0.5, 0.5]; 2^f by a degree-3 polynomial (relative minimax fit, max error 7.5e-5 in fp32 Horner,
-// far inside the 1e-3 score tolerance); 2^n by adding n to the exponent field.
-constexpr float kP0 = 0.9999281168f, kP1 = 0.6932609677f, kP2 = 0.2426105440f, kP3 = 0.0551713221f;
-__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& a, float& b) {
-  float xa, xb;
-  upk2(x2, xa, xb);
-  xa = fmaxf(xa, -125.f); xb = fmaxf(xb, -125.f);          // below fp32's normal range: 2^-125 stands in for 0
-  const uint64_t xc = pk2(xa, xb);
-  const uint64_t t2 = add2(xc, pk2(kMagic, kMagic));         // low mantissa bits = round(x)
-  const uint64_t n2 = add2(t2, pk2(-kMagic, -kMagic));       // round(x) as a float, exact
-  const uint64_t f2 = fma2(n2, pk2(-1.f, -1.f), xc);         // x - round(x), exact
-  uint64_t p2 = fma2(pk2(kP3, kP3), f2, pk2(kP2, kP2));
-  p2 = fma2(p2, f2, pk2(kP1, kP1));
-  p2 = fma2(p2, f2, pk2(kP0, kP0));
-  float pa, pb, ta, tb;
-  upk2(p2, pa, pb);
-  upk2(t2, ta, tb);
-  a = __int_as_float(__float_as_int(pa) + (__float_as_int(ta) << 23));
-  b = __int_as_float(__float_as_int(pb) + (__float_as_int(tb) << 23));
 }
 // 2^d for d <= 0 built from the exponent field; 0 for d <= -127 (such weights are below fp32's range)
 __device__ __forceinline__ float pow2i(int d) { return __int_as_float(max(d + 127, 0) << 23); }

@@ -47,6 +47,7 @@ SYMBOLS = {
     "kara_status": (_i, [_vp, C.POINTER(C.c_int32)]),
     "kara_last_launch_count": (_i, [_vp]),
     "kara_last_score_path": (_i, [_vp]),
+    "kara_last_score_path_reason": (C.c_char_p, [_vp]),
     "kara_enable_score_timing": (_i, [_vp, _i]),
     "kara_score_kernel_ms": (C.c_float, [_vp]),
     "kara_last_error": (C.c_char_p, []),
@@ -269,6 +270,9 @@ class KaraCache:
 
     def last_score_path(self) -> int:
         return int(lib().kara_last_score_path(self._h))
+
+    def last_score_path_reason(self) -> str:
+        return lib().kara_last_score_path_reason(self._h).decode()
 
     def enable_score_timing(self, enable: bool = True) -> None:
         _check(lib().kara_enable_score_timing(self._h, int(enable)))
