@@ -95,7 +95,7 @@ def algorithmic(shape, L, qbuf_only=False):
 # captures of exactly these commands (profiles/r2_ncu_score.md), keyed by (workload, resident layers, variant).
 NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40, "full"): 257.957e6 + 4.504e6, ("cfg3", 8, "full"): 3212.377e6 + 20.670e6,
                            ("cfg4", 2, "full"): 6435.954e6 + 30.069e6, ("cfg5", 8, "full"): 4827.730e6 + 32.882e6,
-                           ("cfg4", 2, "qbuf_only"): 1733.738e6 + 19.043e6}
+                           ("cfg4", 2, "qbuf_only"): 1229.311e6 + 19.162e6}
 NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_score.md (ncu --set full, dram rd+wr of one score-kernel launch of this workload)"
 
 

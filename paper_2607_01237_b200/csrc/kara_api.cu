@@ -239,6 +239,14 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
   k.P = alpha / (gamma - 2);
   k.alpha = alpha; k.gamma = gamma;
   k.q_row_begin = (flags & KARA_SCORE_QBUF_ONLY) ? W - U : 0;
+  k.q_tile_toks = 128; k.q_hpt_log2 = 0;
+  if (flags & KARA_SCORE_QBUF_ONLY) {
+    // pack the U buffer tokens of 2^x heads into one 128-row tile: tokens per tile = largest power of two <= min(U, 128)
+    int tt = 1;
+    while (tt * 2 <= U && tt * 2 <= 128) tt *= 2;
+    k.q_tile_toks = tt;
+    while ((tt << k.q_hpt_log2) < 128) ++k.q_hpt_log2;
+  }
   if ((flags & KARA_SCORE_QBUF_ONLY) && U == 0)
     return fail(KARA_EINVAL, "KARA_SCORE_QBUF_ONLY needs U > 0");
   k.block_table = block_table;

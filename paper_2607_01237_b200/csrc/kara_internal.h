@@ -26,6 +26,9 @@ struct Call {
   int n_windows;    // NW >= 1 disjoint windows of W tokens per sequence (prefill, App. C.2; 1 = the decoding-time step)
   int n_q_heads, G, W, U, n, keep, k, P, alpha, gamma;
   int q_row_begin;  // first window token used as a query (0, or W-U with KARA_SCORE_QBUF_ONLY)
+  // a 128-row query tile of the tcgen05 kernel = q_tile_toks window tokens x (1 << q_hpt_log2) query heads of the group
+  // (128 x 1 normally; with KARA_SCORE_QBUF_ONLY the few buffer tokens of several heads share a tile)
+  int q_tile_toks, q_hpt_log2;
   int32_t* block_table;
   int32_t* seq_lens;
   const int32_t* win_start;

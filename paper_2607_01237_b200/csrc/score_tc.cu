@@ -4,7 +4,8 @@
 //
 // Decomposition.  A unit is one (layer, sequence, KV head).  A query tile is 128 window tokens x
 // ONE query head of the GQA group (rows of a row-softmax are independent, so any (token, head) ->
-// row map is valid; TMA reads the rows at stride n_q_heads*d).  All T = units * tiles_per_unit
+// row map is valid; TMA reads the rows at stride n_q_heads*d); with KARA_SCORE_QBUF_ONLY the U buffer
+// tokens of several heads share a tile (box = tokens x heads, rows past the head group weigh 0).  All T = units * tiles_per_unit
 // tiles of the launch form one sequence that is cut into n_clusters contiguous, equally long
 // ranges (perfect balance; a range crosses unit boundaries, the part of a unit inside a range is
 // a "segment").  A thread-block cluster of CL CTAs owns a range; CTA r of the cluster owns the
@@ -301,12 +302,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           const int stage = q_iter % QS, use = q_iter / QS;
           mbar_wait_backoff(qempty + 8 * stage, (use & 1) ^ 1);
           mbar_expect_tx(qfull + 8 * stage, SM::kQStageBytes);
+          // tile -> (head tile gq, token tile tt): rows = q_tile_toks tokens x 2^q_hpt_log2 heads (token-major in the box)
           const int gq = tile / tok_tiles, tt = tile % tok_tiles;
-          const int tok = ((cur.li * c.n_seqs + cur.s) * c.n_windows + cur.w) * c.W + c.q_row_begin + tt * kTileM;
+          const int tok = ((cur.li * c.n_seqs + cur.s) * c.n_windows + cur.w) * c.W + c.q_row_begin + tt * c.q_tile_toks;
 #pragma unroll
           for (int p = 0; p < SM::kPanels; ++p)
             tma_load_3d(sQ + stage * SM::kQStageBytes + p * (kTileM * 128), &q_map, qfull + 8 * stage,
-                        p * 64, cur.hk * c.G + gq, tok);
+                        p * 64, cur.hk * c.G + (gq << c.q_hpt_log2), tok);
         }
       }
       __syncwarp();
@@ -395,8 +397,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         continue;
       }
       const int n_pieces = (it.n_cols + 31) >> 5;                       // 1 .. 8
-      int tt = it.t0 % tok_tiles;                                       // token tile of `tile` (kept incrementally: no division per tile)
-      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter, tt = (tt + 1 == tok_tiles ? 0 : tt + 1)) {
+      int tt = it.t0 % tok_tiles, gq = it.t0 / tok_tiles;               // token tile / head tile of `tile` (kept incrementally: no division per tile)
+      for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter, gq += (tt + 1 == tok_tiles), tt = (tt + 1 == tok_tiles ? 0 : tt + 1)) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
         KARA_TRACE(3 + (q == 1), tile_iter, 0);
         mbar_wait(bdone + 8 * b, par);                      // every B warp has written e back and left (z, l) per (row, piece)
@@ -448,13 +450,16 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
             }
             z_row = Z; l_row = L;
           }
-          const int tok = c.q_row_begin + tt * kTileM + q * 32 + lane;
+          // tile row r = token r >> hpt_log2 of the tile, head r & (hpt - 1) of the head tile
+          const int r = q * 32 + lane;
+          const int tok = c.q_row_begin + tt * c.q_tile_toks + (r >> c.q_hpt_log2);
+          const bool head_ok = (gq << c.q_hpt_log2) + (r & ((1 << c.q_hpt_log2) - 1)) < c.G;
           // 1 / L on the FMA pipe (a MUFU.RCP would queue behind the B warps' exponentials): the exponent-flip
           // estimate (12 % off at most) and three Newton steps, relative error < 1e-7
           float inv_row = __int_as_float(0x7EF311C7 - __float_as_int(l_row));
 #pragma unroll
           for (int nr = 0; nr < 3; ++nr) inv_row = inv_row * fmaf(-l_row, inv_row, 2.f);
-          if (!(l_row > 0.f) || tok >= c.W) inv_row = 0.f;   // rows past the window contribute nothing
+          if (!(l_row > 0.f) || tok >= c.W || !head_ok) inv_row = 0.f;   // rows past the window / the head group contribute nothing
           // the weights of (row, piece cq of half 0 / half 1) go over the entry as the pairs {w0, w0, w1, w1}
 #pragma unroll
           for (int x = 0; x < 4; ++x) {
@@ -630,8 +635,9 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
   // per launch: the attribute belongs to the current device / context, not to the process
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kAlloc) != cudaSuccess)
     return tc_fail(KARA_ECUDA, "cudaFuncSetAttribute(max dynamic smem) failed");
-  const int tok_tiles = (c.W - c.q_row_begin + kTileM - 1) / kTileM;
-  const int tpu = tok_tiles * c.G;
+  const int tok_tiles = (c.W - c.q_row_begin + c.q_tile_toks - 1) / c.q_tile_toks;
+  const int hpt = 1 << c.q_hpt_log2;
+  const int tpu = tok_tiles * ((c.G + hpt - 1) / hpt);
   const int units = unit_count(c);
   const long long T = (long long)units * tpu;
   if (T >= (1ll << 31)) return tc_fail(KARA_EUNSUPPORTED, "more than 2^31 query tiles in one call");
@@ -721,14 +727,14 @@ const char* score_tc_unsupported_reason(const ScoreTcState& s, const Call& c) {
 bool score_tc_supported(const ScoreTcState& s, const Call& c) { return score_tc_unsupported_reason(s, c) == nullptr; }
 
 int score_tc_launch(ScoreTcState* s, Call& c, cudaStream_t st, int* n_launches) {
-  // window_q tensor map: [d][n_q_heads][layers*seqs*W tokens], box 64 x 1 x 128, 128B swizzle
-  const long long key[6] = {(long long)(uintptr_t)c.window_q, c.g.d, c.n_q_heads, (long long)c.n_layers * c.n_seqs * c.n_windows * c.W, 0, 0};
+  // window_q tensor map: [d][n_q_heads][layers*seqs*W tokens], box 64 x heads-per-tile x tokens-per-tile (= 128 rows), 128B swizzle
+  const long long key[6] = {(long long)(uintptr_t)c.window_q, c.g.d, c.n_q_heads, (long long)c.n_layers * c.n_seqs * c.n_windows * c.W, c.q_tile_toks, c.q_hpt_log2};
   if (s->q_ptr != c.window_q || memcmp(key, s->q_key, sizeof key) != 0) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return tc_fail(KARA_ECUDA, "cuTensorMapEncodeTiled entry point not found");
     cuuint64_t dims[3] = {(cuuint64_t)c.g.d, (cuuint64_t)c.n_q_heads, (cuuint64_t)key[3]};
     cuuint64_t strides[2] = {(cuuint64_t)c.g.d * 2, (cuuint64_t)c.g.d * 2 * c.n_q_heads};
-    cuuint32_t box[3] = {64u, 1u, (cuuint32_t)kTileM};
+    cuuint32_t box[3] = {64u, (cuuint32_t)(1 << c.q_hpt_log2), (cuuint32_t)c.q_tile_toks};   // 128 rows: tokens x heads
     cuuint32_t estr[3] = {1u, 1u, 1u};
     CUtensorMap m;
     CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<__nv_bfloat16*>(c.window_q), dims, strides,

@@ -96,3 +96,26 @@ def test_header_constants_match_the_binding(kara):
             assert getattr(kara, name) == int(val), name
             checked += 1
     assert checked >= 10
+
+
+def test_new_entry_points_check_their_arguments_on_the_host(kara):
+    """kara_compress_windows, kara_policy_step / _commit and kara_window_queries validate their arguments before any CUDA
+    call: errors are codes + messages, never crashes (no GPU needed)."""
+    L = kara.lib()
+    h = L.kara_init_cache(16, 2, 2, 64)
+    assert L.kara_compress_windows(h, 0, 1, 1, 1, 1, 1, None, 0, 1, 4, 64, 8, 0.2, 4, 4, 0, 1, 0, None) == kara.KARA_EINVAL
+    assert b"n_windows" in L.kara_last_error()
+    # policy calls need an attached pool / non-null state
+    assert L.kara_policy_step(h, 4, 1, 8, 1, 1, None, 1, 8, 64, 2, 1, 1, 1, 1, 1, 1, None) == kara.KARA_EINVAL
+    assert b"attach" in L.kara_last_error() or b"pool" in L.kara_last_error()
+    assert L.kara_policy_commit(h, 2, None, None, None, None, None, 64, 8, 0.2, None, 8, None, None, None) == kara.KARA_EINVAL
+    assert L.kara_policy_commit(h, 2, 1, 1, 1, 1, 1, 64, 80, 0.2, 1, 8, 1, 1, None) == kara.KARA_EINVAL     # W <= U
+    L.kara_destroy(h)
+    # the producer: shapes it does not take, alignment, missing workspace for the rotary tables
+    assert L.kara_window_queries(None, None, None, 0, 1e4, 4, 64, 2, 64, None, None, 0, None) == kara.KARA_EINVAL
+    assert L.kara_window_queries(16, 16, None, 0, 1e4, 4, 64, 2, 96, 16, None, 0, None) == kara.KARA_EUNSUPPORTED
+    assert L.kara_window_queries(16, 16, None, 0, 1e4, 4, 100, 2, 64, 16, None, 0, None) == kara.KARA_EUNSUPPORTED
+    assert L.kara_window_queries(16, 24, None, 0, 1e4, 4, 64, 2, 64, 16, None, 0, None) == kara.KARA_EINVAL      # alignment
+    assert L.kara_window_queries(16, 16, 16, 100, 1e4, 4, 64, 2, 64, 16, None, 0, None) == kara.KARA_EINVAL      # no workspace
+    assert L.kara_window_queries_workspace_bytes(131071, 128) == 8 * ((131071 >> 8) + 1 + 256) * 64
+    assert L.kara_window_queries_workspace_bytes(100, 96) == 0
