@@ -62,5 +62,27 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return SO
 
 
+def build_variant(extra_flags, out: Path) -> Path:
+    """Compiles every csrc/*.cu with FLAGS + extra_flags into a scratch directory next to `out` and links them to `out`
+    (a diagnostic build, e.g. -DKARA_TC_DEBUG: the mbarrier watchdog; the product library in-tree is not touched)."""
+    out = Path(out)
+    objdir = out.parent / (out.stem + "_obj")
+    objdir.mkdir(parents=True, exist_ok=True)
+    objs = []
+    for cu in sorted(CSRC.glob("*.cu")):
+        o = objdir / (cu.stem + ".o")
+        r = subprocess.run([NVCC, *FLAGS, *extra_flags, "-c", str(cu), "-o", str(o)], capture_output=True, text=True)
+        if r.returncode:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError(f"nvcc failed on {cu.name}")
+        objs.append(o)
+    r = subprocess.run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static",
+                        *map(str, objs), "-o", str(out)], capture_output=True, text=True)
+    if r.returncode:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("link failed")
+    return out
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

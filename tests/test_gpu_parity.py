@@ -566,3 +566,23 @@ def test_buffer_only_queries_full_parity(gpu, oracle, shape_name):
     nfree = int(Hs["fc"][0])
     np.testing.assert_array_equal(out["fl"][:nfree], Hs["fl"][:nfree])
     print(f"qbuf-only {shape_name}: {n_amb} of {2 * sh.n_seqs * sh.n_kv_heads} units ambiguous")
+
+
+def test_mbarrier_watchdog_build(gpu, chk, tmp_path, monkeypatch):
+    """compute-sanitizer is closed on this GPU pool, so the synchronisation of the score kernel is exercised with the
+    watchdog build instead (-DKARA_TC_DEBUG: every mbarrier wait that does not complete within 2^26 polls traps): the
+    diagnostic library is compiled into a scratch directory, loaded in place of the product library, and must give the
+    oracle's results on shapes that use clusters of 2 and 4, a ragged window start and a multi-window call."""
+    kara, gu = gpu
+    from paper_2607_01237_b200 import build
+    so = build.build_variant(["-DKARA_TC_DEBUG"], tmp_path / "libkara_watchdog.so")
+    monkeypatch.setattr(kara, "_SO", so)
+    monkeypatch.setattr(kara, "_LIB", None)
+    kara.lib()
+    for shape, seed in ((kin.scaled(kin.CFG2, n_layers=2, hist_lo=4099, hist_hi=4099), 2),
+                        (kin.scaled(kin.CFG4, n_seqs=2, n_layers=1, hist_lo=50, hist_hi=400, pool_slack=1.1), 4),
+                        (kin.scaled(kin.CFG1, n_seqs=2, n_layers=2, n_q_heads=4, n_kv_heads=2, n_windows=3, hist_lo=5,
+                                    hist_hi=40), 6)):
+        stats, _, _ = _parity(gpu, chk, kin.generate(shape, seed=seed))
+        assert stats["score_path"] == 2 and stats["s3_hard_mismatch"] == 0
+    monkeypatch.setattr(kara, "_LIB", None)          # the next test loads the product library again
