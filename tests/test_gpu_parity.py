@@ -523,7 +523,7 @@ def test_large_block_sizes(gpu, chk, bs, W, U, d, G, hist):
     assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
 
 
-@pytest.mark.parametrize("shape_name", ["cfg2", "cfg4"])
+@pytest.mark.parametrize("shape_name", ["cfg2", "cfg4", "odd_u40", "odd_u5_g3"])
 def test_buffer_only_queries_full_parity(gpu, oracle, shape_name):
     """KARA_SCORE_QBUF_ONLY ('w/o Bi-Attention') at the cfg2 / cfg4 shapes: the U = 32 buffer rows are the
     last quarter of a 128-row tile, d = 128, clusters of 2 / 4 CTAs.  S1: scores against kara_oracle_scores_buffer_queries on
@@ -532,8 +532,14 @@ def test_buffer_only_queries_full_parity(gpu, oracle, shape_name):
     kara, gu = gpu
     from oracle import check
     from oracle import kara_oracle as ko
-    base = kin.CFG2 if shape_name == "cfg2" else kin.CFG4
-    shape = kin.scaled(base, n_seqs=2, n_layers=2, hist_lo=130, hist_hi=700, pool_slack=1.2)
+    if shape_name == "odd_u40":      # buffer not a power of two: two token tiles, the second 8 / 32 full; 3 heads in a 4-head tile
+        shape = kin.scaled(kin.CFG2, n_seqs=2, n_layers=2, n_q_heads=6, n_kv_heads=2, W=200, U=40, alpha=8, hist_lo=30,
+                           hist_hi=300)
+    elif shape_name == "odd_u5_g3":  # tiny buffer: 4 tokens x 32 heads per tile, 5 tokens -> two token tiles; d = 64
+        shape = kin.scaled(kin.CFG1, n_seqs=3, n_layers=2, n_q_heads=6, n_kv_heads=2, W=69, U=5, hist_lo=3, hist_hi=90)
+    else:
+        base = kin.CFG2 if shape_name == "cfg2" else kin.CFG4
+        shape = kin.scaled(base, n_seqs=2, n_layers=2, hist_lo=130, hist_hi=700, pool_slack=1.2)
     wl = kin.generate(shape, seed=41)
     sh = wl.shape
     H0 = check.host_image(wl)
