@@ -217,6 +217,39 @@ int kara_window_queries(const void* hidden /*dev*/, const void* wq /*dev*/, cons
                         int max_position, double rope_theta, int n_tokens, int d_model, int n_q_heads, int head_dim,
                         void* window_q_out /*dev*/, void* workspace /*dev*/, size_t workspace_bytes, void* stream);
 
+/* kara_window_queries for callers that cannot bring a workspace: the rotary cos / sin tables go into an array that is part
+ * of libkara's own device image instead of into caller memory.  Everything else — arguments, layouts, arithmetic, kernels,
+ * result bits — is kara_window_queries.
+ *
+ * Who needs it.  The producer runs inside a compression event in the middle of decoding.  A serving engine has by then
+ * given every byte of HBM that was left after the weights to its paged KV pool, so a cudaMalloc at that point fails; where
+ * it would still succeed it stalls the whole device while the driver maps memory, which no other stream's decode step can
+ * afford; and engines that route all device memory through one pool (so that usage stays accountable) do not let a
+ * library call the CUDA allocator behind their back.  Such a caller may also have no spare pool buffer to lend for the
+ * few hundred KB of tables.  This entry point calls no cudaMalloc, cudaFree or other allocating routine, ever.
+ *
+ * The limit.  The array is KARA_STATIC_SCRATCH_BYTES (1 MiB) and every GPU on which the process uses libkara carries it from
+ * the moment the library's device code is loaded there until the process exits.  The tables take
+ * kara_window_queries_workspace_bytes(max_position, head_dim) bytes, so max_position <= 458,751 fits at head_dim 128 and
+ * <= 983,039 at head_dim 64.  A larger max_position is refused with KARA_ENOMEM before anything is launched (the message
+ * names the bytes needed and the limit); use kara_window_queries with your own workspace then.
+ *
+ * First call on a device.  The array's device address is looked up (cudaGetSymbolAddress) the first time the entry point
+ * is called with a given device current, and remembered per device; a failure of that lookup is returned as KARA_ECUDA.
+ * Make that first call during start-up, outside any stream capture.  Later calls on that device do no set-up.
+ *
+ * Sharing.  There is one array per GPU and every call on that GPU uses it.  Nothing in it has to start at zero and nothing
+ * is carried from call to call: each call rewrites, on `stream`, every table row its own GEMM epilogue reads (for its own
+ * theta, head_dim and max_position) before that kernel runs, and the previous call's tables are simply overwritten.  The
+ * price is that two calls whose kernels can overlap on the GPU — different streams, or different host threads without an
+ * event between them — race on the tables and may rotate with each other's angles.  Issue the calls of one GPU on one
+ * stream or order them with events.  positions == NULL (no rotary embedding) touches no scratch at all.
+ * Asynchronous on `stream`. */
+#define KARA_STATIC_SCRATCH_BYTES 1048576
+int kara_window_queries_static(const void* hidden /*dev*/, const void* wq /*dev*/, const int32_t* positions /*dev or NULL*/,
+                               int max_position, double rope_theta, int n_tokens, int d_model, int n_q_heads,
+                               int head_dim, void* window_q_out /*dev*/, void* stream);
+
 /* Synchronous: reads and clears the device status word (0 = no fault).  The word is sticky: it holds the
  * OR of the faults of every kara_compress_window call on this handle since the last kara_status(), as long
  * as those calls used the same workspace (the layer-range flow: several calls, KARA_COMMIT on the last). */

@@ -110,6 +110,15 @@ int check_geometry(const kara_cache* c, int layer_begin, int layer_end, int n_se
 
 }  // namespace
 
+// kara_last_error's message, for the translation units that hold an ABI entry point of their own
+int kara::api_fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
 extern "C" {
 
 const char* kara_last_error(void) { return g_err; }

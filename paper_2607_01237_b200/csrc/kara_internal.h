@@ -135,6 +135,9 @@ __device__ inline long long row_offset(const Call& c, int layer, int s, int hk, 
          (long long)(pos & (c.g.bs - 1)) * c.g.d;
 }
 
+// sets the thread-local message kara_last_error() returns and hands `code` back (kara_api.cu)
+int api_fail(int code, const char* fmt, ...);
+
 // kernel launchers (each returns the cudaError_t of its launch)
 cudaError_t launch_score_simt(const Call& c, cudaStream_t st);
 cudaError_t launch_select_compact(const Call& c, cudaStream_t st);

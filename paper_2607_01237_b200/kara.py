@@ -22,6 +22,7 @@ KARA_COMMIT, KARA_KEEP_DEBUG, KARA_SCORE_QBUF_ONLY, KARA_SCORE_SIMT = 1, 2, 4, 8
 (KARA_DBG_K_LOGICAL, KARA_DBG_V_LOGICAL, KARA_DBG_SCORES, KARA_DBG_IDX_TOPK, KARA_DBG_IDX_FINAL,
  KARA_DBG_BLOCK_TABLE_ROW, KARA_DBG_FREE_LIST) = range(7)
 KARA_ST_BAD_BLOCK, KARA_ST_SHORT_SEQ, KARA_ST_TABLE_OVERFLOW, KARA_ST_FREE_OVERFLOW = 1, 2, 4, 8
+KARA_STATIC_SCRATCH_BYTES = 1048576
 
 # every symbol include/kara.h declares: (restype, argtypes)
 _vp, _i, _i64, _sz, _d, _u = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_double, C.c_uint
@@ -43,6 +44,7 @@ SYMBOLS = {
     "kara_policy_commit": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp, _i, _i, _d, _vp, _i, _vp, _vp, _vp]),
     "kara_window_queries_workspace_bytes": (_sz, [_i, _i]),
     "kara_window_queries": (_i, [_vp, _vp, _vp, _i, _d, _i, _i, _i, _i, _vp, _vp, _sz, _vp]),
+    "kara_window_queries_static": (_i, [_vp, _vp, _vp, _i, _d, _i, _i, _i, _i, _vp, _vp]),
     "kara_gather_debug": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i, _vp, _i64, C.POINTER(_i64)]),
     "kara_status": (_i, [_vp, C.POINTER(C.c_int32)]),
     "kara_last_launch_count": (_i, [_vp]),
@@ -108,6 +110,25 @@ def kara_window_queries(hidden: torch.Tensor, wq: torch.Tensor, positions: torch
     st = (stream or torch.cuda.current_stream(hidden.device)).cuda_stream
     _check(lib().kara_window_queries(_ptr(hidden), _ptr(wq), _ptr(positions), max_position or 0, float(rope_theta), T, Dm,
                                      n_q_heads, head_dim, _ptr(out), _ptr(ws), ws.numel() if ws is not None else 0, st))
+    return out
+
+
+def kara_window_queries_static(hidden: torch.Tensor, wq: torch.Tensor, positions: torch.Tensor | None, rope_theta: float,
+                               n_q_heads: int, head_dim: int, out: torch.Tensor, max_position: int,
+                               stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+    """kara_window_queries_static: kara_window_queries without a workspace, for callers that must not allocate device memory
+    during decoding (the rotary tables go into libkara's built-in 1 MiB device array; see include/kara.h for the limit on
+    max_position, the first-call set-up and why calls on one GPU must not overlap).  This binding allocates nothing either:
+    `out` [T, Hq, d] bf16 and `max_position` are the caller's, nothing is read back from the device."""
+    T, Dm = hidden.shape
+    assert hidden.is_cuda and hidden.is_contiguous() and hidden.dtype == torch.bfloat16
+    assert wq.shape == (n_q_heads * head_dim, Dm) and wq.is_contiguous() and wq.dtype == torch.bfloat16
+    assert out.is_cuda and out.is_contiguous() and out.dtype == torch.bfloat16 and out.numel() == T * n_q_heads * head_dim
+    if positions is not None:
+        assert positions.dtype == torch.int32 and positions.is_cuda and positions.numel() == T
+    st = (stream or torch.cuda.current_stream(hidden.device)).cuda_stream
+    _check(lib().kara_window_queries_static(_ptr(hidden), _ptr(wq), _ptr(positions), int(max_position), float(rope_theta), T,
+                                            Dm, n_q_heads, head_dim, _ptr(out), st))
     return out
 
 

@@ -119,3 +119,18 @@ def test_new_entry_points_check_their_arguments_on_the_host(kara):
     assert L.kara_window_queries(16, 16, 16, 100, 1e4, 4, 64, 2, 64, 16, None, 0, None) == kara.KARA_EINVAL      # no workspace
     assert L.kara_window_queries_workspace_bytes(131071, 128) == 8 * ((131071 >> 8) + 1 + 256) * 64
     assert L.kara_window_queries_workspace_bytes(100, 96) == 0
+
+
+def test_static_scratch_entry_point_refuses_oversized_tables_on_the_host(kara):
+    """kara_window_queries_static (no device allocation: rotary tables in the library's built-in array) rejects a
+    max_position whose tables exceed KARA_STATIC_SCRATCH_BYTES before any CUDA call, with the limit in the message."""
+    L = kara.lib()
+    for d, limit in ((128, 458751), (64, 983039)):
+        assert L.kara_window_queries_workspace_bytes(limit, d) == kara.KARA_STATIC_SCRATCH_BYTES
+        rc = L.kara_window_queries_static(16, 16, 16, limit + 1, 1e4, 4, 64, 2, d, 16, None)
+        assert rc == kara.KARA_ENOMEM
+        msg = L.kara_last_error().decode()
+        assert str(kara.KARA_STATIC_SCRATCH_BYTES) in msg and str(limit) in msg and "kara_window_queries" in msg
+    # without positions no scratch is involved: the call is the workspace variant's, argument checks included
+    assert L.kara_window_queries_static(None, None, None, 0, 1e4, 4, 64, 2, 64, None, None) == kara.KARA_EINVAL
+    assert L.kara_window_queries_static(16, 16, None, 0, 1e4, 4, 64, 2, 96, 16, None) == kara.KARA_EUNSUPPORTED
