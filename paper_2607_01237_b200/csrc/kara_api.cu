@@ -68,11 +68,33 @@ int budget(int n, double ratio) {
   return (int)std::ceil(ratio * (double)n - 1e-9);   // reading G5
 }
 
-// tiles_per_unit: query tiles of 128 rows x one head (full-window queries: an upper bound for
-// KARA_SCORE_QBUF_ONLY, whose strip count has the same bound because T shrinks with tpu)
-WsLayout ws_layout(int units, int n, int k, int keep, int tiles_per_unit) {
+// KARA_SCORE_QBUF_ONLY packs the U buffer tokens of 2^x query heads into one 128-row tile: tokens per tile = the largest
+// power of two <= min(U, 128), heads per tile = 128 / that.
+void qbuf_tiling(int U, int* tile_toks, int* hpt_log2) {
+  int tt = 1, l = 0;
+  while (tt * 2 <= U && tt * 2 <= 128) tt *= 2;
+  while ((tt << l) < 128) ++l;
+  *tile_toks = tt;
+  *hpt_log2 = l;
+}
+
+// Query tiles per unit of the two score variants: full window (128 rows x one head) and, if U > 0, buffer queries only.
+// The packed variant can have MORE tiles per unit than the full one (W = 100, U = 65, G = 3: 2 token tiles x 2 head
+// tiles = 4 against 3), so the workspace reserves strips for whichever needs more and serves either flag.
+void tiles_per_unit(int W, int U, int G, int* full, int* qbuf) {
+  *full = (W + 127) / 128 * G;
+  *qbuf = 0;
+  if (U > 0) {
+    int tt, l;
+    qbuf_tiling(U, &tt, &l);
+    *qbuf = (U + tt - 1) / tt * ((G + (1 << l) - 1) >> l);
+  }
+}
+
+WsLayout ws_layout(int units, int n, int k, int keep, int tpu_full, int tpu_qbuf) {
   WsLayout w{};
-  w.parts = strips_bound(units, tiles_per_unit);
+  w.parts = strips_bound(units, tpu_full);
+  if (tpu_qbuf > 0 && strips_bound(units, tpu_qbuf) > w.parts) w.parts = strips_bound(units, tpu_qbuf);
   w.n_pad = round_up(n, 4);
   w.k_pad = round_up(k > 0 ? k : 1, 4);
   w.keep_pad = round_up(keep > 0 ? keep : 1, 4);
@@ -200,7 +222,9 @@ size_t kara_workspace_bytes(const kara_cache* c, int n_layers_in_call, int n_seq
   const int keep = budget(n, ratio);
   if (keep < 0) return 0;
   const int units = n_layers_in_call * n_seqs * c->g.n_kv_heads;
-  return ws_layout(units, n, keep - alpha, keep, (W + 127) / 128 * (n_q_heads / c->g.n_kv_heads)).total;
+  int tpu_full, tpu_qbuf;
+  tiles_per_unit(W, U, n_q_heads / c->g.n_kv_heads, &tpu_full, &tpu_qbuf);
+  return ws_layout(units, n, keep - alpha, keep, tpu_full, tpu_qbuf).total;
 }
 
 int kara_compress_window(kara_cache* c, int layer_begin, int layer_end, int n_seqs, int32_t* block_table,
@@ -229,7 +253,9 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
   const int nL = layer_end - layer_begin;
   const int n = W - U;
   const int units = nL * n_seqs * n_windows * c->g.n_kv_heads;
-  const WsLayout w = ws_layout(units, n, keep - alpha, keep, (W + 127) / 128 * (n_q_heads / c->g.n_kv_heads));
+  int tpu_full, tpu_qbuf;
+  tiles_per_unit(W, U, n_q_heads / c->g.n_kv_heads, &tpu_full, &tpu_qbuf);
+  const WsLayout w = ws_layout(units, n, keep - alpha, keep, tpu_full, tpu_qbuf);
   if (workspace_bytes < w.total)
     return fail(KARA_ENOMEM, "workspace %zu bytes < %zu needed", workspace_bytes, w.total);
 
@@ -250,11 +276,7 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
   k.q_row_begin = (flags & KARA_SCORE_QBUF_ONLY) ? W - U : 0;
   k.q_tile_toks = 128; k.q_hpt_log2 = 0;
   if (flags & KARA_SCORE_QBUF_ONLY) {
-    // pack the U buffer tokens of 2^x heads into one 128-row tile: tokens per tile = largest power of two <= min(U, 128)
-    int tt = 1;
-    while (tt * 2 <= U && tt * 2 <= 128) tt *= 2;
-    k.q_tile_toks = tt;
-    while ((tt << k.q_hpt_log2) < 128) ++k.q_hpt_log2;
+    qbuf_tiling(U, &k.q_tile_toks, &k.q_hpt_log2);
   }
   if ((flags & KARA_SCORE_QBUF_ONLY) && U == 0)
     return fail(KARA_EINVAL, "KARA_SCORE_QBUF_ONLY needs U > 0");
@@ -484,7 +506,7 @@ int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, co
   if (!sel_ids || !sel_count || !sel_block_table || !sel_seq_lens || !sel_win_start || !block_table || !seq_lens ||
       !uncompressed)
     return fail(KARA_EINVAL, "kara_policy_commit: null pointer argument");
-  KARA_CUDA(launch_policy_commit(max_select, max_blocks, keep, U, sel_ids, sel_count, sel_block_table, sel_seq_lens,
+  KARA_CUDA(launch_policy_commit(max_select, max_blocks, keep, U, W, sel_ids, sel_count, sel_block_table, sel_seq_lens,
                                  sel_win_start, block_table, seq_lens, uncompressed,
                                  reinterpret_cast<cudaStream_t>(stream)));
   return KARA_OK;

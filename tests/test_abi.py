@@ -134,3 +134,16 @@ def test_static_scratch_entry_point_refuses_oversized_tables_on_the_host(kara):
     # without positions no scratch is involved: the call is the workspace variant's, argument checks included
     assert L.kara_window_queries_static(None, None, None, 0, 1e4, 4, 64, 2, 64, None, None) == kara.KARA_EINVAL
     assert L.kara_window_queries_static(16, 16, None, 0, 1e4, 4, 64, 2, 96, 16, None) == kara.KARA_EUNSUPPORTED
+
+
+def test_workspace_reserves_strips_for_the_packed_buffer_tiles(kara):
+    """KARA_SCORE_QBUF_ONLY can cut a unit into more query tiles than the full window has (W = 100, U = 65, G = 3: 4 against
+    3), and with few units every tile is a cluster of its own: kara_workspace_bytes must reserve 4 partial-score strips per
+    unit.  2 units, n = 35 (padded to 36), k = 3, keep = 7: status 256 + partial 4 B x 2 x 4 x 36 = 1152 -> 1280 +
+    scores 288 -> 512 + I 256 + F 256 bytes."""
+    L = kara.lib()
+    h = L.kara_init_cache(16, 1, 2, 64)
+    assert L.kara_workspace_bytes(h, 1, 1, 6, 100, 65, 0.2, 4) == 256 + 1280 + 512 + 256 + 256
+    # where the packed variant has fewer tiles nothing changes: 2 units x 1 strip bound by the full window's 3 tiles
+    assert L.kara_workspace_bytes(h, 1, 1, 6, 100, 5, 0.2, 4) == 256 + 4 * 2 * 3 * 96 + 768 + 256 + 256
+    L.kara_destroy(h)
