@@ -81,7 +81,12 @@ extern "C" {
 #define KARA_ST_BAD_BLOCK 1   /* a block-table entry touched by the window is outside [0, num_blocks) */
 #define KARA_ST_SHORT_SEQ 2   /* win_start < 0 or win_start + W > seq_len */
 #define KARA_ST_TABLE_OVERFLOW 4 /* ceil(seq_len / block_size) > max_blocks */
-#define KARA_ST_FREE_OVERFLOW 8  /* a5 would push past free_list[num_blocks) (stale or duplicated free_count) */
+#define KARA_ST_FREE_OVERFLOW 8  /* a5 would push past free_list[num_blocks) (stale, negative or duplicated free_count): the
+                                    K/V rows are already compacted at that point, so seq_lens and the block tables ARE
+                                    committed (they must describe the rows as they now lie), but the blocks the step frees
+                                    are dropped instead of pushed and free_count does not move — per group of 256 sequences
+                                    in batch order.  The cache stays consistent; the blocks leak until the caller rebuilds
+                                    its free list.  (The other three bits skip the sequence as a whole.) */
 
 typedef struct kara_cache kara_cache;
 
@@ -193,7 +198,9 @@ int kara_policy_step(kara_cache* c, int n_seqs, int32_t* block_table /*dev, in/o
 
 /* Alg. 1 l.12 UpdateMetadata(e) for the running queue after the sub-batch was compressed and committed: for x < *sel_count,
  * s = sel_ids[x]: block_table[s][:] = sel_block_table[x][:], seq_lens[s] = sel_seq_lens[x], and uncompressed[s] = U + t with
- * t = sel_seq_lens[x] - (sel_win_start[x] + keep + U), keep = ceil(ratio (W-U)).  Asynchronous on `stream`. */
+ * t = sel_seq_lens[x] - (sel_win_start[x] + keep + U), keep = ceil(ratio (W-U)).  A row whose sel_seq_lens[x] still equals
+ * seq_lens[s] although keep + U < W was skipped by kara_compress_window (a fault in its status word): nothing of that
+ * sequence is committed, it stays eligible.  Asynchronous on `stream`. */
 int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, const int32_t* sel_count,
                        const int32_t* sel_block_table, const int32_t* sel_seq_lens, const int32_t* sel_win_start,
                        int W, int U, double ratio, int32_t* block_table /*dev*/, int max_blocks,

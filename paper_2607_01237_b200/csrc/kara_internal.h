@@ -148,7 +148,7 @@ cudaError_t launch_policy_step(int n_seqs, int max_blocks, int bs, int bs_log2, 
                                int32_t* free_list, int32_t* free_count, int32_t* step_counter, int32_t* sel_ids,
                                int32_t* sel_count, int32_t* sel_block_table, int32_t* sel_seq_lens, int32_t* sel_win_start,
                                int32_t* exhausted, cudaStream_t st);
-cudaError_t launch_policy_commit(int max_select, int max_blocks, int keep, int U, const int32_t* sel_ids,
+cudaError_t launch_policy_commit(int max_select, int max_blocks, int keep, int U, int W, const int32_t* sel_ids,
                                  const int32_t* sel_count, const int32_t* sel_block_table, const int32_t* sel_seq_lens,
                                  const int32_t* sel_win_start, int32_t* block_table, int32_t* seq_lens,
                                  int32_t* uncompressed, cudaStream_t st);

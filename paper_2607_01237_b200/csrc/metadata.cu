@@ -59,18 +59,20 @@ __global__ void __launch_bounds__(kThreads) metadata_kernel(const Call c) {
       tot += warp_tot[w];
     }
     base += inc - freed;
-    // a stale or duplicated free_count must not push past the list: the whole batch of 256 sequences is refused
-    // (uniform decision, so the running count stays consistent) and the status word says why
+    // A stale or duplicated free_count must not push past the list.  By now a4 has already compacted the rows of these
+    // sequences, so refusing the commit would leave seq_lens and the tables describing rows that no longer exist:
+    // the lengths and tables ARE committed, but the trailing blocks of this group of 256 sequences are dropped instead
+    // of pushed (they leak until the caller rebuilds its free list), free_count does not move, and the status word
+    // says why.  The decision is uniform over the group, so the running count stays consistent.
     const bool overflow = (long long)s_running + tot > c.g.num_blocks || s_running < 0;
     if (overflow) {
       if (tid == 0) atomicOr(c.status, KARA_ST_FREE_OVERFLOW);
-      ok = false;
       tot = 0;
     }
     if (ok) {
       int32_t* row = c.block_table + (long long)s * c.max_blocks;
       for (int b = new_nb; b < old_nb; ++b) {
-        c.free_list[base + (b - new_nb)] = row[b];
+        if (!overflow) c.free_list[base + (b - new_nb)] = row[b];
         row[b] = -1;
       }
       c.seq_lens[s] = new_len;

@@ -120,24 +120,33 @@ __global__ void __launch_bounds__(kThreads) policy_step_kernel(const PolicyArgs 
 }
 
 struct CommitArgs {
-  int max_select, max_blocks, keep, U;
+  int max_select, max_blocks, keep, U, W;
   const int32_t* sel_ids; const int32_t* sel_count; const int32_t* sel_block_table; const int32_t* sel_seq_lens;
   const int32_t* sel_win_start;
   int32_t* block_table; int32_t* seq_lens; int32_t* uncompressed;
 };
 
 __global__ void __launch_bounds__(kThreads) policy_commit_kernel(const CommitArgs a) {
+  __shared__ int s_skip;
   const int cnt = min(*a.sel_count, a.max_select);
   for (int x = 0; x < cnt; ++x) {
     const int s = a.sel_ids[x];
     if (s < 0) continue;
-    for (int b = threadIdx.x; b < a.max_blocks; b += kThreads)
-      a.block_table[(long long)s * a.max_blocks + b] = a.sel_block_table[(long long)x * a.max_blocks + b];
-    if (threadIdx.x == 0) {
-      const int len = a.sel_seq_lens[x];
-      a.seq_lens[s] = len;
-      a.uncompressed[s] = a.U + (len - (a.sel_win_start[x] + a.keep + a.U));   // buffer + tail stay uncompressed
+    // A sub-batch row that kara_compress_window skipped (a fault recorded in its status word) comes back with the length
+    // it went in with — a compressed one is shorter by W - keep - U > 0 tokens.  Such a sequence was not compressed:
+    // its table row, length and uncompressed count stay as they are (it is still eligible at the next event).
+    if (threadIdx.x == 0) s_skip = (a.sel_seq_lens[x] == a.seq_lens[s] && a.keep + a.U < a.W) ? 1 : 0;
+    __syncthreads();
+    if (!s_skip) {
+      for (int b = threadIdx.x; b < a.max_blocks; b += kThreads)
+        a.block_table[(long long)s * a.max_blocks + b] = a.sel_block_table[(long long)x * a.max_blocks + b];
+      if (threadIdx.x == 0) {
+        const int len = a.sel_seq_lens[x];
+        a.seq_lens[s] = len;
+        a.uncompressed[s] = a.U + (len - (a.sel_win_start[x] + a.keep + a.U));   // buffer + tail stay uncompressed
+      }
     }
+    __syncthreads();
   }
 }
 
@@ -155,11 +164,11 @@ cudaError_t launch_policy_step(int n_seqs, int max_blocks, int bs, int bs_log2, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_policy_commit(int max_select, int max_blocks, int keep, int U, const int32_t* sel_ids,
+cudaError_t launch_policy_commit(int max_select, int max_blocks, int keep, int U, int W, const int32_t* sel_ids,
                                  const int32_t* sel_count, const int32_t* sel_block_table, const int32_t* sel_seq_lens,
                                  const int32_t* sel_win_start, int32_t* block_table, int32_t* seq_lens,
                                  int32_t* uncompressed, cudaStream_t st) {
-  CommitArgs a{max_select, max_blocks, keep, U, sel_ids, sel_count, sel_block_table, sel_seq_lens, sel_win_start,
+  CommitArgs a{max_select, max_blocks, keep, U, W, sel_ids, sel_count, sel_block_table, sel_seq_lens, sel_win_start,
                block_table, seq_lens, uncompressed};
   policy_commit_kernel<<<1, kThreads, 0, st>>>(a);
   return cudaGetLastError();

@@ -227,10 +227,12 @@ def test_device_status_word_flags_bad_inputs(gpu):
     assert out["status"] & kara.KARA_ST_SHORT_SEQ
 
 
-def test_bad_block_sequence_is_skipped_as_a_whole(gpu, chk):
-    """include/kara.h: a sequence whose window touches a block id outside the pool is skipped before anything is
-    written: its K/V blocks, its block-table row, its seq_len stay byte-identical and nothing of it reaches the
-    free list; the other sequences of the batch come out exactly as the oracle computes them without it."""
+@pytest.mark.parametrize("fault", ["bad_block", "table_overflow"])
+def test_faulty_sequence_is_skipped_as_a_whole(gpu, chk, fault):
+    """include/kara.h: a sequence whose window touches a block id outside the pool (KARA_ST_BAD_BLOCK), or whose length
+    needs more blocks than its table row has (KARA_ST_TABLE_OVERFLOW), is skipped before anything is written: its K/V
+    blocks, its block-table row, its seq_len stay byte-identical and nothing of it reaches the free list; the other
+    sequences of the batch come out exactly as the oracle computes them without it."""
     kara, gu = gpu
     shape = kin.scaled(kin.CFG3, n_seqs=3, n_layers=2, hist_lo=100, hist_hi=700, tail_lo=0, tail_hi=9)
     wl = kin.generate(shape, seed=31)
@@ -238,17 +240,21 @@ def test_bad_block_sequence_is_skipped_as_a_whole(gpu, chk):
     bad_s = 1
     h, ln = int(wl.win_start[bad_s]), int(wl.seq_lens[bad_s])
     D = gu.to_cuda(wl)
-    bad_entry = h // bs + 3
-    D["bt"][bad_s, bad_entry] = wl.num_blocks + 5
-    bt_in = D["bt"].cpu().numpy().copy()
+    if fault == "bad_block":
+        D["bt"][bad_s, h // bs + 3] = wl.num_blocks + 5
+        bit = kara.KARA_ST_BAD_BLOCK
+    else:
+        D["sl"][bad_s] = wl.block_table.shape[1] * bs + 1       # one token more than the table row can address
+        bit = kara.KARA_ST_TABLE_OVERFLOW
+    bt_in, sl_in = D["bt"].cpu().numpy().copy(), D["sl"].cpu().numpy().copy()
     for tc_path in (True, False):
         Dr = {k: v.clone() for k, v in D.items()}
         flags = kara.KARA_COMMIT | kara.KARA_KEEP_DEBUG | (0 if tc_path else kara.KARA_SCORE_SIMT)
         out, cache, _ = gu.gpu_compress(wl, dev_tensors=Dr, flags=flags)
-        assert out["status"] & kara.KARA_ST_BAD_BLOCK
+        assert out["status"] == bit
         # the offending sequence: nothing of it changed
         np.testing.assert_array_equal(out["bt"][bad_s], bt_in[bad_s])
-        assert out["sl"][bad_s] == ln
+        assert out["sl"][bad_s] == sl_in[bad_s]
         H0 = chk.host_image(wl)
         own_blocks = [int(b) for b in wl.block_table[bad_s, :(ln + bs - 1) // bs] if 0 <= int(b) < wl.num_blocks]
         np.testing.assert_array_equal(out["k"][:, own_blocks], H0["k"][:, own_blocks])
@@ -268,6 +274,32 @@ def test_bad_block_sequence_is_skipped_as_a_whole(gpu, chk):
         assert np.all((out["fl"][:nfree] >= 0) & (out["fl"][:nfree] < wl.num_blocks))
         np.testing.assert_array_equal(out["k"], Hs["k"])
         np.testing.assert_array_equal(out["v"], Hs["v"])
+
+
+@pytest.mark.parametrize("stale_count", ["full", "negative"])
+def test_free_list_overflow_commits_the_cache_and_drops_the_blocks(gpu, chk, stale_count):
+    """KARA_ST_FREE_OVERFLOW (include/kara.h): with a free_count that leaves no room for the blocks the step frees (a stale
+    count equal to the pool size) or a negative one, a5 runs after a4 has already moved the rows — so the lengths and block
+    tables must still be committed (pools, tables and seq_lens exactly the oracle's), while the freed blocks are dropped:
+    free_list and free_count stay byte-identical to what the caller passed, and the status word carries the bit."""
+    kara, gu = gpu
+    shape = kin.scaled(kin.CFG3, n_seqs=3, n_layers=2, hist_lo=100, hist_hi=700, tail_lo=0, tail_hi=9)
+    wl = kin.generate(shape, seed=33)
+    sh = wl.shape
+    D = gu.to_cuda(wl)
+    D["fc"][0] = wl.num_blocks if stale_count == "full" else -3
+    fl_in, fc_in = D["fl"].cpu().numpy().copy(), D["fc"].cpu().numpy().copy()
+    out, cache, _ = gu.gpu_compress(wl, dev_tensors=D)
+    assert out["status"] == kara.KARA_ST_FREE_OVERFLOW
+    Hs = chk.host_image(wl)                       # the oracle on the pristine workload, from the GPU's scores (stage S2)
+    assert (Hs["sl"] > 0).all()
+    chk.run_oracle(Hs, sh.n_q_heads, sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma, 0, 2, True,
+                   scores_in=np.ascontiguousarray(out["scores"], np.float32))
+    for key in ("k", "v", "bt", "sl"):
+        np.testing.assert_array_equal(out[key], Hs[key], err_msg=key)
+    assert int(Hs["fc"][0]) > int(chk.host_image(wl)["fc"][0])        # the step does free blocks: there was something to drop
+    np.testing.assert_array_equal(out["fl"], fl_in)
+    np.testing.assert_array_equal(out["fc"], fc_in)
 
 
 def test_status_word_is_sticky_across_layer_range_calls(gpu):
@@ -523,7 +555,7 @@ def test_large_block_sizes(gpu, chk, bs, W, U, d, G, hist):
     assert stats["s3_hard_mismatch"] == 0 and stats["score_path"] == 2
 
 
-@pytest.mark.parametrize("shape_name", ["cfg2", "cfg4", "odd_u40", "odd_u5_g3"])
+@pytest.mark.parametrize("shape_name", ["cfg2", "cfg4", "odd_u40", "odd_u5_g3", "odd_u65_w100_g3"])
 def test_buffer_only_queries_full_parity(gpu, oracle, shape_name):
     """KARA_SCORE_QBUF_ONLY ('w/o Bi-Attention') at the cfg2 / cfg4 shapes: the U = 32 buffer rows are the
     last quarter of a 128-row tile, d = 128, clusters of 2 / 4 CTAs.  S1: scores against kara_oracle_scores_buffer_queries on
@@ -537,6 +569,11 @@ def test_buffer_only_queries_full_parity(gpu, oracle, shape_name):
                            hist_hi=300)
     elif shape_name == "odd_u5_g3":  # tiny buffer: 4 tokens x 32 heads per tile, 5 tokens -> two token tiles; d = 64
         shape = kin.scaled(kin.CFG1, n_seqs=3, n_layers=2, n_q_heads=6, n_kv_heads=2, W=69, U=5, hist_lo=3, hist_hi=90)
+    elif shape_name == "odd_u65_w100_g3":
+        # the packed buffer tiles outnumber the full-window tiles (2 token tiles x 2 head tiles = 4 per unit against
+        # ceil(100/128) x 3 = 3) and the batch is small enough for one tile per cluster: 4 strips per unit, which the
+        # workspace of kara_workspace_bytes has to hold (it once reserved 3 and the call failed with KARA_ENOMEM)
+        shape = kin.scaled(kin.CFG1, n_seqs=1, n_layers=2, n_q_heads=6, n_kv_heads=2, W=100, U=65, hist_lo=11, hist_hi=11)
     else:
         base = kin.CFG2 if shape_name == "cfg2" else kin.CFG4
         shape = kin.scaled(base, n_seqs=2, n_layers=2, hist_lo=130, hist_hi=700, pool_slack=1.2)

@@ -91,3 +91,33 @@ def test_decoding_loop_with_policy_and_compression(oracle, bs, W, U, delta, m, S
         assert exhausted > 0                  # the small pool ran dry: those sequences were not advanced, on both sides
     live = np.concatenate([H["bt"][s][H["bt"][s] >= 0] for s in range(S)])
     assert sorted(np.concatenate([live, H["fl"][: int(H["fc"][0])]]).tolist()) == list(range(NB))
+
+
+def test_policy_commit_leaves_a_skipped_sequence_alone():
+    """kara_policy_commit (include/kara.h): a sub-batch row that kara_compress_window skipped because of a fault comes back
+    with the length it went in with; committing it would set `uncompressed` to U + t as if its window had been compressed.
+    Two selected rows, the first compressed (shorter by W - keep - U), the second returned unchanged: the first sequence
+    takes the sub-batch's table row, length and U + t, the second keeps its table row, length and counter."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_01237_b200 import kara
+    dev = torch.device("cuda:0")
+    W, U, ratio, max_blocks = 64, 8, 0.25, 12
+    keep = kara.kara_budget(W - U, ratio)                         # 14
+    i32 = dict(dtype=torch.int32, device=dev)
+    bt = torch.arange(4 * max_blocks, **i32).reshape(4, max_blocks).contiguous()
+    sl = torch.tensor([150, 90, 170, 40], **i32)
+    un = torch.tensor([70, 66, 75, 40], **i32)
+    # sequences 2 and 1 were selected, in that order; window starts 100 and 20, tails t = 170-100-64 = 6 and 90-20-64 = 6
+    sel = dict(ids=torch.tensor([2, 1, -1], **i32), count=torch.tensor([2], **i32),
+               block_table=torch.full((3, max_blocks), -7, **i32), win_start=torch.tensor([100, 20, 0], **i32),
+               seq_lens=torch.tensor([170 - (W - keep - U), 90, -1], **i32))
+    bt0, sl0, un0 = bt.clone(), sl.clone(), un.clone()
+    h = kara.KaraCache(16, 1, 1, 64)
+    h.policy_commit(sel, W, U, ratio, bt, sl, un)
+    torch.cuda.synchronize()
+    assert sl.tolist() == [150, 90, 170 - (W - keep - U), 40]
+    assert un.tolist() == [70, 66, U + 6, 40]
+    assert (bt[2] == -7).all()
+    for s in (0, 1, 3):
+        assert torch.equal(bt[s], bt0[s])
