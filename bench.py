@@ -97,6 +97,19 @@ NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40, "full"): 257.957e6 + 4.504e6, ("cfg3", 8
                            ("cfg4", 2, "full"): 6435.954e6 + 30.069e6, ("cfg5", 8, "full"): 4827.730e6 + 32.882e6,
                            ("cfg4", 2, "qbuf_only"): 1229.311e6 + 19.162e6}
 NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_score.md (ncu --set full, dram rd+wr of one score-kernel launch of this workload)"
+# The captures were taken at this commit; the number is only reported while the score kernel's sources are still the
+# ones of that commit (sha256 over the files below, in this order) — otherwise `traffic` is null and `traffic_stale` true.
+NCU_TRAFFIC_COMMIT = "26d0175"
+SCORE_KERNEL_SOURCES = ("score_tc.cu", "score_tc_ptx.cuh", "score_tc.h")
+SCORE_KERNEL_SHA256_AT_CAPTURE = "da4c9a44f8c004536a9a29b17fc193dce58d21183fec50ffa82626c4276ec6fc"
+
+
+def score_kernel_sha256():
+    import hashlib
+    h = hashlib.sha256()
+    for f in SCORE_KERNEL_SOURCES:
+        h.update((ROOT / "paper_2607_01237_b200" / "csrc" / f).read_bytes())
+    return h.hexdigest()
 
 
 def _peaks():
@@ -213,7 +226,7 @@ def oracle_all_cores(workload, L_per_proc):
 
 
 # layers of one sequence per oracle pass: about 10-30 s of CPU work on one core
-ORACLE_LAYERS = {"cfg1": 1, "cfg2": 24, "cfg3": 24, "cfg4": 6, "cfg5": 2, "prefill": 2}
+ORACLE_LAYERS = {"cfg1": 1, "cfg2": 24, "cfg3": 24, "cfg4": 8, "cfg5": 2, "prefill": 2}   # cfg4: 8 layers x 8 heads = 64 units
 ORACLE_LAYERS_PER_PROC = {"cfg1": 1, "cfg2": 8, "cfg3": 8, "cfg4": 2, "cfg5": 1, "prefill": 1}
 
 
@@ -241,8 +254,13 @@ def run_reference(args):
 
 # -------------------------------------------------------------------------------------------------
 def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False, qbuf_only=False, alpha0=False,
-            score_timing=True, want_e2e=False):
-    """Generates workload `name` on `dev`, times `steps` steps (after `warmup`) and returns the raw numbers."""
+            score_timing=True, want_e2e=False, ratio=None, per_layer_calls=False, also_without_events=False):
+    """Generates workload `name` on `dev`, times `steps` steps (after `warmup`) and returns the raw numbers.
+    ratio: retention override (BASELINE.json configs[3] sweeps 10 / 20 / 30 %).  per_layer_calls: the step is one
+    kara_compress_window call PER LAYER (KARA_COMMIT on the last), the way Alg. 1 l.6-12 interleaves with the model's
+    layers, instead of one call over all resident layers.  also_without_events: `steps` more steps with the library's
+    event pair around the score launch switched off (the select kernel is launched programmatically behind the score
+    kernel; an event record between the two sits where that overlap happens)."""
     import torch
     from paper_2607_01237_b200 import inputs as kin
     from paper_2607_01237_b200 import kara
@@ -251,6 +269,8 @@ def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False,
     shape = _shape(name)
     if alpha0:
         shape = kin.scaled(shape, alpha=0)                   # "w/o Token2Chunk"
+    if ratio is not None:
+        shape = kin.scaled(shape, ratio=ratio)
     L = _resident_layers(name, shape, L_req)
     NW = shape.n_windows
     seed = replicas.rank_seed(SEEDS[name], rank)
@@ -288,7 +308,12 @@ def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False,
         torch.cuda.synchronize()
 
     def step():
-        if NW > 1:
+        if per_layer_calls:
+            for l in range(L):
+                cache.compress_window(l, l + 1, wl.block_table, wl.seq_lens, wl.win_start, wl.window_q[l:l + 1], shape.W,
+                                      shape.U, shape.ratio, shape.alpha, shape.gamma,
+                                      flags if l == L - 1 else flags & ~kara.KARA_COMMIT, workspace=ws)
+        elif NW > 1:
             cache.compress_windows(0, L, wl.block_table, wl.seq_lens, wl.win_start, NW, wl.window_q, shape.W, shape.U,
                                    shape.ratio, shape.alpha, shape.gamma, flags, workspace=ws)
         else:
@@ -322,9 +347,21 @@ def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False,
     if dist:
         dist.barrier()
     torch.cuda.synchronize()
+    launches_step = cache.last_launch_count() if not per_layer_calls else 2 * L + 1   # (score + select) per layer + a5
     res = dict(shape=shape, L=L, total_ms=sum(step_ms), score_ms=sum(score_ms) / len(score_ms), freed=freed,
-               launches=cache.last_launch_count() * steps, score_path=score_path, clocks=clk.summary(),
-               alg=algorithmic(shape, L, qbuf_only), wc_step=shape.n_seqs * NW * L, e2e=None)
+               launches=launches_step * steps, score_path=score_path, clocks=clk.summary(),
+               alg=algorithmic(shape, L, qbuf_only), wc_step=shape.n_seqs * NW * L, e2e=None, ms_no_events=None)
+    if also_without_events:
+        cache.enable_score_timing(False)
+        ms = []
+        for it in range(2 + steps):
+            restore()
+            ev0.record(stream); step(); ev1.record(stream)
+            torch.cuda.synchronize()
+            if it >= 2:
+                ms.append(ev0.elapsed_time(ev1))
+        res["ms_no_events"] = sum(ms) / len(ms)
+        cache.enable_score_timing(score_timing)
 
     # ---- e2e: same step through the host-buffer entry point (pinned host inputs) -------------
     if want_e2e and NW == 1:
@@ -417,7 +454,8 @@ def run_gpu(args):
     variant = "qbuf_only" if args.qbuf_only else "alpha0" if args.alpha0 else "full"
 
     res = measure(args.workload, args.layers, args.steps, args.warmup, dev, rank, dist, local_rank, simt=args.simt,
-                  qbuf_only=args.qbuf_only, alpha0=args.alpha0, score_timing=not args.no_score_timing, want_e2e=True)
+                  qbuf_only=args.qbuf_only, alpha0=args.alpha0, score_timing=not args.no_score_timing, want_e2e=True,
+                  also_without_events=not args.no_score_timing)
     e2e_mean = res["e2e"]["mean_s"] if res["e2e"] else 0.0
     total_ms, e2e_mean = replicas.max_over_ranks([res["total_ms"], e2e_mean], dist, dev)
     shape, L, alg = res["shape"], res["L"], res["alg"]
@@ -434,8 +472,10 @@ def run_gpu(args):
                     "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                     "frac": d["score_tflops"] / peaks["bf16_tflops"] if d["score_tflops"] else None,
                     "flops_per_launch": alg["flops"]}
-    roofline.update({"traffic": NCU_SCORE_TRAFFIC_BYTES.get((args.workload, L, variant)),
-                     "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peaks["source"] + ", burst",
+    stale = score_kernel_sha256() != SCORE_KERNEL_SHA256_AT_CAPTURE
+    roofline.update({"traffic": None if stale else NCU_SCORE_TRAFFIC_BYTES.get((args.workload, L, variant)),
+                     "traffic_source": NCU_TRAFFIC_SOURCE, "traffic_capture_commit": NCU_TRAFFIC_COMMIT,
+                     "traffic_stale": stale, "peak_source": peaks["source"] + ", burst",
                      "kernel_ms": d["score_ms"], "share_of_step": d["score_ms"] / d["ms_per_step"]})
     line = {
         "metric": METRIC, "value": d["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -450,6 +490,9 @@ def run_gpu(args):
                  "api": "kara_compress_window_host (pinned host window_q/tables in, tables + free count out)"}
                 if res["e2e"] else None),
         "gpu_launches": res["launches"],
+        # the same step with the library's two event records around the score launch switched off (they sit between the
+        # score kernel and the select kernel that is launched programmatically behind it); rank 0's mean, same protocol
+        "ms_per_step_no_score_events": res["ms_no_events"],
         "roofline": roofline,
         "step_roofline": {"t_tensor_ms": d["t_tensor_ms"], "t_hbm_ms": d["t_hbm_ms"], "frac": d["step_frac"],
                           "def": "slower of (algorithmic bytes / measured HBM GB/s) and (score FLOPs / measured bf16 TFLOP/s) over ms_per_step"},
@@ -467,6 +510,29 @@ def run_gpu(args):
                          "roofline_frac": dd["score_tflops"] / peaks["bf16_tflops"], "score_kernel_ms": dd["score_ms"],
                          "step_roofline_frac": dd["step_frac"], "freed_blocks_per_step": r["freed"],
                          "gpu_launches": r["launches"], "sm_mhz": r["clocks"]["sm_mhz"]}
+        # BASELINE.json configs[3]: retention swept over 10 / 20 / 30 % with the freed-block counts (SURVEY 8(d) expects
+        # about 55.75 / 49.56 / 43.38 freed blocks per sequence); the headline above is the 20 % point
+        for pct in (10, 30):
+            if args.workload != "cfg4":
+                break
+            r = measure("cfg4", 0, 5, 3, dev, rank, None, local_rank, ratio=pct / 100)
+            dd = derived(r, peaks, 1, None, 5)
+            per[f"cfg4_r{pct}"] = {"workload": _workload_label("cfg4", r["shape"]) + f", retention {pct} %",
+                                   "n_layers": r["L"], "steps": 5, "ms_per_step": dd["ms_per_step"], "value": dd["value"],
+                                   "roofline_frac": dd["score_tflops"] / peaks["bf16_tflops"],
+                                   "score_kernel_ms": dd["score_ms"], "step_roofline_frac": dd["step_frac"],
+                                   "freed_blocks_per_step": r["freed"],
+                                   "freed_blocks_per_sequence": r["freed"] / r["shape"].n_seqs,
+                                   "gpu_launches": r["launches"], "sm_mhz": r["clocks"]["sm_mhz"]}
+        # SURVEY 8(d) timing protocol: cfg 2 also as one call PER LAYER (8 units per call: the latency case of Alg. 1
+        # l.6-12) beside the one all-layer call above
+        r = measure("cfg2", 0, 5, 3, dev, rank, None, local_rank, per_layer_calls=True, score_timing=False)
+        per["cfg2_per_layer_calls"] = {"workload": _workload_label("cfg2", r["shape"]) + ", one call per layer",
+                                       "n_layers": r["L"], "calls_per_step": r["L"], "steps": 5,
+                                       "ms_per_step": r["total_ms"] / 5, "us_per_call": 1e3 * r["total_ms"] / 5 / r["L"],
+                                       "value": r["wc_step"] / (r["total_ms"] / 5 * 1e-3),
+                                       "freed_blocks_per_step": r["freed"], "gpu_launches": r["launches"],
+                                       "sm_mhz": r["clocks"]["sm_mhz"]}
         per["window_q_producer"] = measure_producer(dev, peaks)
         line["per_config"] = per
     if rank == 0:
