@@ -227,6 +227,8 @@ int qproj_launch(const void* hidden, const void* wq, const int32_t* positions, i
   if (positions) {
     if (workspace_bytes < qproj_workspace_bytes(max_position, d)) return q_fail(KARA_ENOMEM, "workspace too small for the rotary tables");
     rope_tables_kernel<<<64, 256, 0, st>>>(theta, d, n_hi, tab_hi, tab_lo);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return q_fail(KARA_ECUDA, cudaGetErrorString(e));
   }
   CUtensorMap amap, bmap;
   cuuint32_t estr[2] = {1u, 1u};
