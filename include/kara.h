@@ -215,9 +215,13 @@ int kara_policy_commit(kara_cache* c, int max_select, const int32_t* sel_ids, co
  * states (the layer's normalised inputs, i.e. everything before the projection) are the caller's.
  *   hidden        [dev bf16 n_tokens x d_model]   d_model a multiple of 64; 16-byte aligned
  *   wq            [dev bf16 (n_q_heads*head_dim) x d_model]
- *   positions     [dev int32 n_tokens] in [0, max_position], or NULL: no rotary embedding
+ *   positions     [dev int32 n_tokens] in [0, max_position], or NULL: no rotary embedding.  The range is the CALLER'S
+ *                 contract: there is no device-side check and no status word on this call — a position outside it is
+ *                 rotated by the angle of some position inside it (the table index is clamped), i.e. wrongly and silently
  *   window_q_out  [dev bf16 n_tokens x n_q_heads x head_dim]  (tokens in the order of the call's window_q: sequence, token)
- *   workspace     [dev] >= kara_window_queries_workspace_bytes(max_position, head_dim) (cos / sin tables; unused without positions)
+ *   workspace     [dev] >= kara_window_queries_workspace_bytes(max_position, head_dim) (cos / sin tables; unused without positions).
+ *                 The tables are rebuilt on `stream` by every call (a few microseconds), so calls that may overlap on the GPU
+ *                 must not share a workspace
  * Asynchronous on `stream`.  One hand-written tcgen05 / TMA GEMM with the rotary embedding fused into its epilogue. */
 size_t kara_window_queries_workspace_bytes(int max_position, int head_dim);
 int kara_window_queries(const void* hidden /*dev*/, const void* wq /*dev*/, const int32_t* positions /*dev or NULL*/,
@@ -258,8 +262,9 @@ int kara_window_queries_static(const void* hidden /*dev*/, const void* wq /*dev*
                                int head_dim, void* window_q_out /*dev*/, void* stream);
 
 /* Synchronous: reads and clears the device status word (0 = no fault).  The word is sticky: it holds the
- * OR of the faults of every kara_compress_window call on this handle since the last kara_status(), as long
- * as those calls used the same workspace (the layer-range flow: several calls, KARA_COMMIT on the last). */
+ * OR of the faults of every kara_compress_window(s) call on this handle since the last kara_status() (or since
+ * kara_attach_pool, which clears it) — whatever workspaces those calls used.  It lives in device memory that belongs to
+ * the library (a slot of a static array, one per live handle, at most 4096 handles), not in the workspace. */
 int kara_status(kara_cache* c, int32_t* status_out /*host*/);
 
 /* Number of kernel launches the last kara_compress_window call made (for bench.py's gpu_launches). */

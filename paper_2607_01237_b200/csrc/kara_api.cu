@@ -5,12 +5,20 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "kara_internal.h"
 #include "score_tc.h"
 
 using namespace kara;
+
+// The device status words (include/kara.h, kara_status) live in the library's own device image, one 32-byte slot per live
+// handle, NOT in the caller's workspace: a workspace may be freed and handed out again at the same address with garbage in
+// it, or be shared by two handles, and neither may turn into fault bits or erase another handle's.  No allocation: the
+// array is part of every GPU's copy of the module; a handle looks its slot's address up when a pool is attached.
+constexpr int kMaxHandles = 4096;
+static __device__ __align__(32) int32_t g_status_slots[kMaxHandles][8];
 
 struct kara_cache {
   Geom g{};
@@ -25,9 +33,9 @@ struct kara_cache {
   int last_launches = 0;
   int last_score_path = 0;
   const char* last_score_reason = "";   // why the CUDA-core kernel ran ("" when the tcgen05 kernel did)
-  // sticky device status word: not cleared between the calls of a step (see kara_status)
-  const void* status_ws = nullptr;
-  bool status_pending = false;
+  // sticky device status word: g_status_slots[status_slot] on the device of the attached pool (see kara_status)
+  int status_slot = -1;
+  int32_t* status_dev = nullptr;
   // score-kernel timing
   bool timing = false;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -56,6 +64,21 @@ int fail(int code, const char* fmt, ...) {
     cudaError_t e__ = (expr);                                                            \
     if (e__ != cudaSuccess) return fail(KARA_ECUDA, "%s: %s", #expr, cudaGetErrorString(e__)); \
   } while (0)
+
+std::mutex g_slot_mutex;
+bool g_slot_used[kMaxHandles] = {};
+
+int take_status_slot() {
+  std::lock_guard<std::mutex> lock(g_slot_mutex);
+  for (int i = 0; i < kMaxHandles; ++i)
+    if (!g_slot_used[i]) { g_slot_used[i] = true; return i; }
+  return -1;
+}
+void release_status_slot(int i) {
+  if (i < 0) return;
+  std::lock_guard<std::mutex> lock(g_slot_mutex);
+  g_slot_used[i] = false;
+}
 
 int ilog2_exact(int x) {
   int l = 0;
@@ -163,6 +186,12 @@ kara_cache* kara_init_cache(int block_size, int n_layers, int n_kv_heads, int he
   }
   kara_cache* c = new (std::nothrow) kara_cache();
   if (!c) { fail(KARA_ENOMEM, "host allocation failed"); return nullptr; }
+  c->status_slot = take_status_slot();
+  if (c->status_slot < 0) {
+    delete c;
+    fail(KARA_ENOMEM, "more than %d live handles (kara_destroy the ones no longer used)", kMaxHandles);
+    return nullptr;
+  }
   c->g.bs = block_size;
   c->g.bs_log2 = l2;
   c->g.n_layers = n_layers;
@@ -182,6 +211,7 @@ void kara_destroy(kara_cache* c) {
   if (c->d_sl) cudaFree(c->d_sl);
   if (c->d_ws) cudaFree(c->d_ws);
   if (c->d_work) cudaFree(c->d_work);
+  release_status_slot(c->status_slot);
   delete c;
 }
 
@@ -206,8 +236,13 @@ int kara_attach_pool(kara_cache* c, void* k_pool, void* v_pool, int64_t num_bloc
   c->free_count = free_count;
   c->g.num_blocks = num_blocks;
   c->g.sL = c->g.sB * num_blocks;
-  c->attached = true;
   c->have_last = false;
+  // this handle's status slot on the current device (the pool's), cleared: a destroyed handle may have left bits in it
+  void* slots = nullptr;
+  KARA_CUDA(cudaGetSymbolAddress(&slots, g_status_slots));
+  c->status_dev = static_cast<int32_t*>(slots) + (size_t)c->status_slot * 8;
+  KARA_CUDA(cudaMemset(c->status_dev, 0, 8 * sizeof(int32_t)));
+  c->attached = true;
   int rc = score_tc_attach(&c->tc, c->g, k_pool);
   if (rc != KARA_OK) return fail(rc, "TMA descriptor for the K pool: %s", score_tc_error());
   return KARA_OK;
@@ -285,7 +320,7 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
   k.win_start = win_start;
   k.window_q = static_cast<const __nv_bfloat16*>(window_q);
   char* base = static_cast<char*>(workspace);
-  k.status = reinterpret_cast<int32_t*>(base + w.status_off);
+  k.status = c->status_dev;          // library-owned, sticky until kara_status (the workspace's first 32 bytes are unused)
   k.partial = reinterpret_cast<float*>(base + w.partial_off);
   k.scores = reinterpret_cast<float*>(base + w.scores_off);
   k.idx_topk = reinterpret_cast<int32_t*>(base + w.topk_off);
@@ -297,11 +332,6 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
   k.free_list = c->free_list;
   k.free_count = c->free_count;
 
-  // the status word accumulates over the calls of a step (same workspace) until kara_status() reads it
-  if (!(c->status_pending && c->status_ws == workspace))
-    KARA_CUDA(cudaMemsetAsync(k.status, 0, 8 * sizeof(int32_t), st));
-  c->status_ws = workspace;
-  c->status_pending = true;
   int launches = 0;
 
   // ---- a1 score ------------------------------------------------------------------------------
@@ -537,11 +567,10 @@ int kara_window_queries(const void* hidden, const void* wq, const int32_t* posit
 int kara_status(kara_cache* c, int32_t* status_out) {
   if (!c || !status_out) return fail(KARA_EINVAL, "null argument");
   *status_out = 0;
-  if (!c->have_last) return KARA_OK;
+  if (!c->status_dev) return KARA_OK;       // no pool attached yet: nothing can have faulted
   KARA_CUDA(cudaDeviceSynchronize());
-  KARA_CUDA(cudaMemcpy(status_out, c->last.status, sizeof(int32_t), cudaMemcpyDeviceToHost));
-  KARA_CUDA(cudaMemset(c->last.status, 0, sizeof(int32_t)));
-  c->status_pending = false;
+  KARA_CUDA(cudaMemcpy(status_out, c->status_dev, sizeof(int32_t), cudaMemcpyDeviceToHost));
+  KARA_CUDA(cudaMemset(c->status_dev, 0, 8 * sizeof(int32_t)));
   return KARA_OK;
 }
 

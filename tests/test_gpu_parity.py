@@ -323,6 +323,31 @@ def test_status_word_is_sticky_across_layer_range_calls(gpu):
     assert cache.status() == 0                              # read-and-clear
 
 
+def test_status_word_does_not_live_in_the_workspace(gpu):
+    """kara_status: the word belongs to the handle (library-owned device memory), so a workspace that comes with garbage in
+    it — a caching allocator handing the same address out again — sets no bits, and a second handle working in the same
+    workspace neither sees nor erases the first handle's fault."""
+    kara, gu = gpu
+    wl = kin.generate(kin.scaled(kin.CFG1, n_layers=2), seed=3)
+    sh = wl.shape
+    A, B = gu.to_cuda(wl), gu.to_cuda(wl)
+    caches = []
+    for D in (A, B):
+        c = kara.KaraCache(sh.block_size, 2, sh.n_kv_heads, sh.head_dim)
+        c.attach_pool(D["k"], D["v"], D["fl"], D["fc"])
+        caches.append(c)
+    ws = torch.full((caches[0].workspace_bytes(2, sh.n_seqs, sh.n_q_heads, sh.W, sh.U, sh.ratio, sh.alpha),), 0xFF,
+                    dtype=torch.uint8, device="cuda")
+    A["bt"][0, 17] = wl.num_blocks + 5
+    for c, D in zip(caches, (A, B)):
+        c.compress_window(0, 2, D["bt"], D["sl"], D["ws"], D["q"], sh.W, sh.U, sh.ratio, sh.alpha, sh.gamma,
+                          kara.KARA_COMMIT, workspace=ws)
+    torch.cuda.synchronize()
+    assert caches[1].status() == 0                              # neither the garbage nor the other handle's fault
+    assert caches[0].status() == kara.KARA_ST_BAD_BLOCK         # still there after the other handle's call and status read
+    assert caches[0].status() == 0
+
+
 def test_argument_errors_are_reported_not_thrown(gpu):
     kara, gu = gpu
     wl = kin.generate(kin.CFG1, seed=1)
