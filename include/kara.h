@@ -66,7 +66,9 @@ extern "C" {
                                     not be freed while other layers still hold live rows in them. */
 #define KARA_KEEP_DEBUG 2u       /* keep scores / I / F of every unit in the workspace for kara_gather_debug */
 #define KARA_SCORE_QBUF_ONLY 4u  /* ablation "w/o Bi-Attention": queries = buffer U only */
-#define KARA_SCORE_SIMT 8u       /* force the CUDA-core score kernel (debug cross-check of the tcgen05 path) */
+#define KARA_SCORE_SIMT 8u       /* run the CUDA-core score kernel (debug cross-check of the tcgen05 path).  It is never
+                                    chosen for you: a call the tcgen05 kernel cannot take (no sm_100 device, a K pool of
+                                    2^31 rows or more, 2^31 window tokens or more) returns KARA_EUNSUPPORTED without it */
 
 /* `what` of kara_gather_debug */
 #define KARA_DBG_K_LOGICAL 0  /* bf16 [seq_len][d] rows of (layer, seq, kv_head) read through the block table */
@@ -272,8 +274,8 @@ int kara_last_launch_count(const kara_cache* c);
 
 /* Which score kernel the last call used: 0 = none yet, 1 = CUDA-core (SIMT), 2 = tcgen05/TMA. */
 int kara_last_score_path(const kara_cache* c);
-/* "" if the tcgen05 kernel ran, else why the CUDA-core kernel did (KARA_SCORE_SIMT, or a shape / device the tcgen05
- * kernel does not take).  The CUDA-core kernel is a cross-check, not a second backend: bench.py refuses its numbers. */
+/* "" if the tcgen05 kernel ran, else why the CUDA-core kernel did (only ever: KARA_SCORE_SIMT was set).  The CUDA-core
+ * kernel is a cross-check, not a second backend: bench.py refuses its numbers. */
 const char* kara_last_score_path_reason(const kara_cache* c);
 
 /* Device time of the score kernel (a1) alone: when enabled, every kara_compress_window call

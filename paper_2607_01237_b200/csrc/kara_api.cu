@@ -335,7 +335,12 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
   int launches = 0;
 
   // ---- a1 score ------------------------------------------------------------------------------
-  const bool use_tc = !(flags & KARA_SCORE_SIMT) && score_tc_supported(c->tc, k);
+  // One score backend: the tcgen05 / TMA kernel.  A call it cannot take is an error, not a quiet detour through the
+  // CUDA-core kernel — that one runs only when the caller asks for it by name (KARA_SCORE_SIMT, a cross-check).
+  if (!(flags & KARA_SCORE_SIMT) && !score_tc_supported(c->tc, k))
+    return fail(KARA_EUNSUPPORTED, "the tcgen05 score kernel cannot take this call (%s); KARA_SCORE_SIMT runs the CUDA-core "
+                "cross-check kernel instead, on purpose", score_tc_unsupported_reason(c->tc, k));
+  const bool use_tc = !(flags & KARA_SCORE_SIMT);
   if (c->timing) {
     if (!c->ev0) { KARA_CUDA(cudaEventCreate(&c->ev0)); KARA_CUDA(cudaEventCreate(&c->ev1)); }
     KARA_CUDA(cudaEventRecord(c->ev0, st));
@@ -355,8 +360,7 @@ int kara_compress_windows(kara_cache* c, int layer_begin, int layer_end, int n_s
     KARA_CUDA(launch_score_simt(k, st));
     ++launches;
     c->last_score_path = 1;
-    // never silent: the reason is kept for kara_last_score_path_reason (bench.py refuses to report such a run)
-    c->last_score_reason = (flags & KARA_SCORE_SIMT) ? "KARA_SCORE_SIMT was set" : score_tc_unsupported_reason(c->tc, k);
+    c->last_score_reason = "KARA_SCORE_SIMT was set";
   }
   if (c->timing) { KARA_CUDA(cudaEventRecord(c->ev1, st)); c->ev_recorded = true; }
 
