@@ -348,6 +348,36 @@ def test_status_word_does_not_live_in_the_workspace(gpu):
     assert caches[0].status() == 0
 
 
+def test_no_silent_detour_through_the_cuda_core_score_kernel(gpu):
+    """north_star: no multi-backend dispatch.  A call the tcgen05 kernel cannot take is refused with KARA_EUNSUPPORTED and
+    the reason; the CUDA-core kernel runs only under KARA_SCORE_SIMT.  The one such call that needs no 500 GB pool: a
+    geometry whose K pool has 2^31 rows (64 layers x 8 heads x block 256 x 16,384 blocks — one tensor map cannot index it)
+    attached over a small buffer, with a batch of one ABSENT row (seq_len -1: skipped before any memory is touched)."""
+    kara, gu = gpu
+    L = kara.lib()
+    h = L.kara_init_cache(256, 64, 8, 128)
+    assert h
+    buf = torch.zeros(1 << 20, dtype=torch.uint8, device="cuda")
+    fl, fc = torch.zeros(16384, dtype=torch.int32, device="cuda"), torch.zeros(1, dtype=torch.int32, device="cuda")
+    assert L.kara_attach_pool(h, buf.data_ptr(), buf.data_ptr(), 16384, fl.data_ptr(), fc.data_ptr()) == kara.KARA_OK
+    bt = torch.full((1, 8), -1, dtype=torch.int32, device="cuda")
+    sl = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+    q = torch.zeros(1, 1, 512, 40, 128, dtype=torch.bfloat16, device="cuda")
+    nbytes = L.kara_workspace_bytes(h, 1, 1, 40, 512, 32, 0.2, 32)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    call = lambda flags: L.kara_compress_window(h, 0, 1, 1, bt.data_ptr(), 8, sl.data_ptr(), None, q.data_ptr(), 40, 512, 32,
+                                                0.2, 32, 8, flags, ws.data_ptr(), nbytes, None)
+    assert call(kara.KARA_COMMIT) == kara.KARA_EUNSUPPORTED
+    msg = L.kara_last_error().decode()
+    assert "tcgen05" in msg and "KARA_SCORE_SIMT" in msg and "2^31" in msg
+    assert L.kara_last_score_path(h) == 0 and L.kara_last_launch_count(h) == 0        # nothing was launched
+    assert call(kara.KARA_COMMIT | kara.KARA_SCORE_SIMT) == kara.KARA_OK
+    torch.cuda.synchronize()
+    assert L.kara_last_score_path(h) == 1 and L.kara_last_score_path_reason(h) == b"KARA_SCORE_SIMT was set"
+    assert int(sl[0]) == -1 and int(fc[0]) == 0
+    L.kara_destroy(h)
+
+
 def test_argument_errors_are_reported_not_thrown(gpu):
     kara, gu = gpu
     wl = kin.generate(kin.CFG1, seed=1)
@@ -521,13 +551,18 @@ def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
     for s in range(S):
         touched[bt0[s, int(h[s]) // bs: int(-(-old_len[s] // bs))].long()] = True
     assert torch.equal(wl.k_pool[:, ~touched], k0[:, ~touched]) and torch.equal(wl.v_pool[:, ~touched], v0[:, ~touched])
-    # every unit: sum_j A_j = G W (sampled over a stride to keep the read-back short), F sorted / unique / in range
-    for u in range(0, L * S * Hkv, 7 if name == "cfg3" else 13):
+    # EVERY unit of the batch: sum_j A_j = G W, and stage S2 of the index work — the oracle's Eq. 5-8 + C.3 on the GPU's own
+    # fp32 scores must give the GPU's I and F bit for bit (microseconds per unit for the oracle)
+    for u in range(L * S * Hkv):
         l, s, hk = u // (S * Hkv), (u // Hkv) % S, u % Hkv
         A = cache.gather_debug(kara.KARA_DBG_SCORES, l, s, hk)
+        I = cache.gather_debug(kara.KARA_DBG_IDX_TOPK, l, s, hk)
         F = cache.gather_debug(kara.KARA_DBG_IDX_FINAL, l, s, hk)
         assert abs(float(A.astype(np.float64).sum()) - G * sh.W) <= 1e-4 * G * sh.W
         assert F.shape[0] == keep and np.all(np.diff(F) > 0) and F[0] >= 0 and F[-1] < n
+        inj = ko.select(A, keep, sh.alpha, sh.gamma)
+        np.testing.assert_array_equal(I, inj["I"], err_msg=f"S2 I of unit {(l, s, hk)}")
+        np.testing.assert_array_equal(F, inj["F"], err_msg=f"S2 F of unit {(l, s, hk)}")
     # a5 on the WHOLE batch: the oracle's metadata step on the pristine tables -> block tables, seq_lens and the free list
     # (order included) must be bit-identical
     bt_o, sl_o = bt0.cpu().numpy().copy(), sl0.cpu().numpy().copy()
@@ -540,7 +575,9 @@ def test_batch_configs_at_scale_sampled_units(gpu, oracle, name, L, ratio):
     # sampled units against the oracle: sequences across the history-length deciles plus the sequences that own the
     # lowest and the highest block id of the pool (both pool ends), layers / heads drawn at random
     rng = np.random.default_rng(11)
-    n_samples = 4 if name == "cfg5" else 16                # (a cfg5 unit is 8.3 GFLOP for the oracle)
+    # >= 64 units per config (cfg4: 16 + 64 + 16 over its three retention points); a cfg5 unit is 8.3 GFLOP
+    # of plain fp64 loops for the oracle (about 2 s), so cfg5 takes one unit of every sequence of its batch of 16
+    n_samples = 16 if name == "cfg5" or (name == "cfg4" and ratio != 0.2) else 64
     order = np.argsort(h, kind="stable")
     picks = [int(order[min(S - 1, (d * S) // max(n_samples - 2, 1))]) for d in range(n_samples - 2)]
     bt_np = bt0.cpu().numpy()
