@@ -101,7 +101,10 @@ NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_score.md (ncu --set full, dram rd+wr of on
 # ones of that commit (sha256 over the files below, in this order) — otherwise `traffic` is null and `traffic_stale` true.
 NCU_TRAFFIC_COMMIT = "26d0175"
 SCORE_KERNEL_SOURCES = ("score_tc.cu", "score_tc_ptx.cuh", "score_tc.h")
-SCORE_KERNEL_SHA256_AT_CAPTURE = "da4c9a44f8c004536a9a29b17fc193dce58d21183fec50ffa82626c4276ec6fc"
+# (sources as of the round-3 clean-up: the trace / diagnostic switches and unused PTX helpers were removed after the capture;
+# `cuobjdump -sass` of score_tc.o is identical instruction for instruction before and after, so the capture still describes
+# this kernel)
+SCORE_KERNEL_SHA256_AT_CAPTURE = "766c3e9f98689d782663db473fe64f64d42b572f55dc1a68844662c106551abe"
 
 
 def score_kernel_sha256():
@@ -451,6 +454,9 @@ def run_gpu(args):
     dev = torch.device(f"cuda:{local_rank}")
     kara.lib()
     peaks = _peaks()
+    if args.producer_only:
+        print(json.dumps({"window_q_producer": measure_producer(dev, peaks, steps=max(args.steps, 1))}))
+        return
     variant = "qbuf_only" if args.qbuf_only else "alpha0" if args.alpha0 else "full"
 
     res = measure(args.workload, args.layers, args.steps, args.warmup, dev, rank, dist, local_rank, simt=args.simt,
@@ -566,6 +572,9 @@ def main():
     ap.add_argument("--alpha0", action="store_true", help="ablation 'w/o Token2Chunk' (PAPER.md:L195): alpha = 0")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config legs (cfg2, cfg3, cfg5, prefill)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--producer-only", action="store_true",
+                    help="time only the window-query producer (kara_window_queries) and print its per_config object; "
+                         "the command to put under ncu for qproj_kernel")
     ap.add_argument("--no-score-timing", action="store_true",
                     help="no CUDA events inside the library around the score launch (roofline.kernel_ms = 0)")
     args = ap.parse_args()

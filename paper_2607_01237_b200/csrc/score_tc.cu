@@ -17,7 +17,7 @@
 //       refilled as soon as its column sums have been taken.
 //   The softmax is split over SPECIALISED warps:
 //   B warps (16: TMEM lane quadrant q x 32-column piece cq of each MMA half) — pass B, the only MUFU work.
-//       One TMEM read, one write, in the 16x32bx2 shape: a THREAD OWNS 32 CONSECUTIVE COLUMNS OF ONE ROW (a "piece",
+//       One TMEM read, one write, in the 32x32b shape (four .x8 loads): a THREAD OWNS 32 CONSECUTIVE COLUMNS OF ONE ROW (a "piece",
 //       one per half), so the maximum, the integer shift z = round(max c) (log2 domain) and the row sum
 //       l = sum 2^(s c - z) are thread-local: no shuffle anywhere in the pass.  e = 2^(s c - z) is written
 //       back in place; (z, l) per (row, 32-column piece) go to shared memory.
@@ -56,15 +56,6 @@ constexpr int kThreads = 32 * 24;             // 6 warpgroups (setmaxnreg works 
 constexpr int kRegsB = 80, kRegsC = 120, kRegsOther = 40;
 thread_local char g_tc_err[256] = "";
 
-#ifdef KARA_TC_TRACE
-// debug build: clock64() stamps of CTA 0's warp roles per tile (see kara_tc_trace_read below)
-constexpr int kTraceTiles = 64, kTraceEv = 8, kTraceRoles = 5;   // roles: 0 = B warp 0, 1 = B warp 15, 2 = MMA, 3 = C warp 16, 4 = C warp 17
-__device__ long long g_trace[kTraceRoles * kTraceTiles * kTraceEv];
-#define KARA_TRACE(role, ti, ev)                                                                     \
-  do { if (blockIdx.x == 0 && lane == 0 && (ti) < kTraceTiles) g_trace[((role) * kTraceTiles + (ti)) * kTraceEv + (ev)] = clock64(); } while (0)
-#else
-#define KARA_TRACE(role, ti, ev) do { } while (0)
-#endif
 
 // ------------------------------------------------------------------------------------------------
 // shared-memory carve-up (dynamic smem, manually aligned to 1024 B for the 128B swizzle)
@@ -161,9 +152,7 @@ __device__ __forceinline__ void pass_b_body(uint32_t (&r)[32], int& z_out, float
   for (int i = 0; i < 16; ++i) {
     float a, b;
     upk2(fma2(pk2(x[2 * i], x[2 * i + 1]), cs2, nz2), a, b);
-#ifndef KARA_DBG_NO_EX2                        // (diagnostic build: what the kernel costs without a single exponential)
     a = ex2(a); b = ex2(b);
-#endif
     if (i & 1) lb = add2(lb, pk2(a, b)); else la = add2(la, pk2(a, b));
     r[2 * i] = __float_as_uint(a); r[2 * i + 1] = __float_as_uint(b);
   }
@@ -340,15 +329,12 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       for (int i = 0; i < n_tiles; ++i, ++q_iter, ++tile_iter) {
         const int stage = q_iter % QS, quse = q_iter / QS;
         const int buf = tile_iter & 1, tuse = tile_iter >> 1;
-        KARA_TRACE(2, tile_iter, 0);
         mbar_wait(qfull + 8 * stage, quse & 1);
-        KARA_TRACE(2, tile_iter, 1);
         const uint32_t a_lo = ((sQ + stage * SM::kQStageBytes) >> 4) | kDescLo;
 #pragma unroll
         for (int hf = 0; hf < 2; ++hf) {
           mbar_wait(tempty + 8 * (buf * 2 + hf), (tuse & 1) ^ 1);
           tc_fence_after();
-          KARA_TRACE(2, tile_iter, 2 + 2 * hf);
           if (elect_one()) {
             const int nc = half_cols(n_cols, hf);
             if (nc > 0) {
@@ -372,7 +358,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
             }
           }
           __syncwarp();
-          KARA_TRACE(2, tile_iter, 3 + 2 * hf);
         }
       }
     }
@@ -400,9 +385,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
       int tt = it.t0 % tok_tiles, gq = it.t0 / tok_tiles;               // token tile / head tile of `tile` (kept incrementally: no division per tile)
       for (int tile = it.t0; tile < it.t1; ++tile, ++tile_iter, gq += (tt + 1 == tok_tiles), tt = (tt + 1 == tok_tiles ? 0 : tt + 1)) {
         const int b = tile_iter & 1, par = (tile_iter >> 1) & 1;
-        KARA_TRACE(3 + (q == 1), tile_iter, 0);
         mbar_wait(bdone + 8 * b, par);                      // every B warp has written e back and left (z, l) per (row, piece)
-        KARA_TRACE(3 + (q == 1), tile_iter, 1);
         // the first TMEM read of pass C is requested now: it lands while the statistics below are merged
         tc_fence_after();
         const uint32_t ta = tq + b * kKeysPerCta, ta_hi = ta + (16u << 16);
@@ -435,9 +418,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
 #pragma unroll
             for (int pr = 0; pr < CL; ++pr)
               if (pr != rank) st_async_b32x2(mapa(la, pr), (uint32_t)z_row, __float_as_uint(l_row), mapa(bar, pr));
-            KARA_TRACE(3 + (q == 1), tile_iter, 2);
             mbar_wait(bar, par);
-            KARA_TRACE(3 + (q == 1), tile_iter, 3);
             // ... and merges that row over the CTAs in rank order (identical bits on every CTA)
             int Z = z_row;
 #pragma unroll
@@ -470,17 +451,12 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
           __syncwarp();
         }
         tc_fence_after();
-        KARA_TRACE(3 + (q == 1), tile_iter, 4);
         // weights: rows lr + 8k (k = 0..3) x pieces 0..7, {w, w} pairs, fetched just before their use
         const uint2* wrow = reinterpret_cast<const uint2*>(rstat + (size_t)(b * 4) * 128 + q * 32 + lr);
         auto wld = [&](int pc, int k) -> uint64_t {        // piece pc = 4 hf + cq in column order
           const uint2 v = wrow[(size_t)((pc & 3) * 128 + 8 * k) * 2 + (pc >> 2)];
           return pk2u(v.x, v.y);
         };
-#ifdef KARA_DBG_NO_C
-        if (lane == 0) { mbar_arrive(tempty + 8 * (b * 2 + 0)); mbar_arrive(tempty + 8 * (b * 2 + 1)); }
-        continue;
-#endif
         // ---- pass C: acc_j += sum_i e_ij w_i, piece by piece (16 rows x 32 columns per TMEM read, the next read in flight
         // under the FFMA2s of the current one); each half is handed back to the MMA warp as soon as it has been read ----
 #define KARA_C_STEP(PC)                                                                   \
@@ -498,13 +474,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 0));
-        KARA_TRACE(3 + (q == 1), tile_iter, 5);
         KARA_C_STEP(4) KARA_C_STEP(5) KARA_C_STEP(6) KARA_C_STEP(7)
 #undef KARA_C_STEP
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + 8 * (b * 2 + 1));
-        KARA_TRACE(3 + (q == 1), tile_iter, 6);
       }
 
       // ---- segment done: combine lanes (fixed order), then the 4 warps (fixed order), write the strip ----
@@ -555,17 +529,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         const uint32_t ta = tq + b * kKeysPerCta;
         int z0 = kZFloor, z1 = kZFloor;
         float l0 = 0.f, l1 = 0.f;
-        const bool trc = (warp == 0 || warp == 15);
         uint32_t ra[32], rb[32];
-        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 0);
         mbar_wait(tfull + 8 * (b * 2 + 0), par);
         tc_fence_after();
         tmem_ld_32x32b_x32(ta, ra);                      // (an inactive piece is loaded too and ignored)
-        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 1);
         // the TMEM load of piece 1 runs under the exponentials of piece 0 (in the B-bound steady state its S half
         // has landed long before; a starved B warp loses at most the time between the two MMA halves here)
         tmem_wait_ld();
-        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 2);
         // ---- pass B: e = 2^(s c - z) in place; (z, l) of (row, piece); the thread owns row 32 q + lane ----
         if (act0) {
           pass_b_piece(ra, z0, l0, cs, colw0, colw_n, pcq * 32, c_lo, c_hi);
@@ -574,19 +544,16 @@ score_tc_kernel(const __grid_constant__ CUtensorMap k_map, const __grid_constant
         mbar_wait(tfull + 8 * (b * 2 + 1), par);
         tc_fence_after();
         tmem_ld_32x32b_x32(ta + kHalf, rb);
-        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 3);
         tmem_wait_ld();
         if (act1) {
           pass_b_piece(rb, z1, l1, cs, kHalf + colw0, colw_n, kHalf + pcq * 32, c_lo, c_hi);
           tmem_st_32x32b_x32(ta + kHalf, rb);
         }
         rstat[(b * 4 + pcq) * 128 + row] = make_uint4((uint32_t)z0, __float_as_uint(l0), (uint32_t)z1, __float_as_uint(l1));
-        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 4);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bdone + 8 * b);
-        if (trc) KARA_TRACE(warp == 0 ? 0 : 1, tile_iter, 5);
       }
     }
   }
@@ -678,12 +645,6 @@ int launch_impl(ScoreTcState* s, Call& c, cudaStream_t st) {
 
 const char* score_tc_error() { return g_tc_err; }
 
-#ifdef KARA_TC_TRACE
-extern "C" int kara_tc_trace_read(long long* out, int n) {
-  if (n > kTraceRoles * kTraceTiles * kTraceEv) n = kTraceRoles * kTraceTiles * kTraceEv;
-  return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * n);
-}
-#endif
 
 int score_tc_attach(ScoreTcState* s, const Geom& g, void* k_pool) {
   s->ready = false;
