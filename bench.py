@@ -257,7 +257,8 @@ def run_reference(args):
 
 # -------------------------------------------------------------------------------------------------
 def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False, qbuf_only=False, alpha0=False,
-            score_timing=True, want_e2e=False, ratio=None, per_layer_calls=False, also_without_events=False):
+            score_timing=True, want_e2e=False, ratio=None, per_layer_calls=False, also_without_events=False,
+            want_chain=False):
     """Generates workload `name` on `dev`, times `steps` steps (after `warmup`) and returns the raw numbers.
     ratio: retention override (BASELINE.json configs[3] sweeps 10 / 20 / 30 %).  per_layer_calls: the step is one
     kara_compress_window call PER LAYER (KARA_COMMIT on the last), the way Alg. 1 l.6-12 interleaves with the model's
@@ -386,6 +387,45 @@ def measure(name, L_req, steps, warmup, dev, rank, dist, local_rank, simt=False,
                 e2e_s.append(dt)
         res["e2e"] = dict(mean_s=sum(e2e_s) / len(e2e_s), h2d=h2d, d2h=d2h)
         del hq
+    # ---- device-resident chain: hidden states -> kara_window_queries -> kara_compress_window, layer by layer -------
+    # What a serving engine runs at a compression event (App. C.2: the window's query states are
+    # recomputed on the device; they never cross PCIe): per resident layer the window-query producer writes window_q[l]
+    # from the layer's hidden states, then that layer is compressed (KARA_COMMIT on the last).  Synthetic hidden states
+    # (one [n_seqs*W, d_model] bf16 buffer shared by the layers) and per-layer random W_q at the model's d_model =
+    # n_q_heads * head_dim; positions = the window tokens' own.  The producer goes through the no-allocation entry point.
+    res["chain"] = None
+    if want_chain and NW == 1:
+        Hq, d = shape.n_q_heads, shape.head_dim
+        Dm, T = Hq * d, shape.n_seqs * shape.W
+        hid = torch.randn(T, Dm, device=dev, dtype=torch.bfloat16)
+        wqs = [(torch.randn(Hq * d, Dm, device=dev, dtype=torch.bfloat16) / Dm ** 0.5) for _ in range(L)]
+        pos = (wl.win_start.view(-1, 1) + torch.arange(shape.W, device=dev, dtype=torch.int32).view(1, -1)).reshape(-1)
+        pos = pos.to(torch.int32).contiguous()
+        max_pos = int(pos.max())
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(L)]
+        cache.enable_score_timing(False)
+        chain_ms, prod_ms = [], []
+        n_chain = max(3, min(steps, 10))
+        for it in range(2 + n_chain):
+            restore()
+            ev0.record(stream)
+            for l in range(L):
+                evs[l][0].record(stream)
+                kara.kara_window_queries_static(hid, wqs[l], pos, 1e6, Hq, d, wl.window_q[l].view(T, Hq, d), max_pos)
+                evs[l][1].record(stream)
+                cache.compress_window(l, l + 1, wl.block_table, wl.seq_lens, wl.win_start, wl.window_q[l:l + 1], shape.W,
+                                      shape.U, shape.ratio, shape.alpha, shape.gamma,
+                                      flags if l == L - 1 else flags & ~kara.KARA_COMMIT, workspace=ws)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            if it >= 2:
+                chain_ms.append(ev0.elapsed_time(ev1))
+                prod_ms.append(sum(evs[l][0].elapsed_time(evs[l][1]) for l in range(L)))
+        assert cache.status() == 0, "device status word set in the chain leg"
+        res["chain"] = dict(ms=sum(chain_ms) / len(chain_ms), producer_ms=sum(prod_ms) / len(prod_ms), steps=n_chain,
+                            hidden_bytes=hid.numel() * 2, d_model=Dm, tokens=T,
+                            producer_flops=2.0 * T * Dm * Hq * d * L, launches=(2 + 2) * L + 1)
+        del hid, wqs, pos
     cache.close()
     del wl, k0, v0, ws, flush, cache
     torch.cuda.empty_cache()
@@ -461,7 +501,7 @@ def run_gpu(args):
 
     res = measure(args.workload, args.layers, args.steps, args.warmup, dev, rank, dist, local_rank, simt=args.simt,
                   qbuf_only=args.qbuf_only, alpha0=args.alpha0, score_timing=not args.no_score_timing, want_e2e=True,
-                  also_without_events=not args.no_score_timing)
+                  also_without_events=not args.no_score_timing, want_chain=True)
     e2e_mean = res["e2e"]["mean_s"] if res["e2e"] else 0.0
     total_ms, e2e_mean = replicas.max_over_ranks([res["total_ms"], e2e_mean], dist, dev)
     shape, L, alg = res["shape"], res["L"], res["alg"]
@@ -495,6 +535,19 @@ def run_gpu(args):
                  "d2h_bytes_per_step": res["e2e"]["d2h"], "ms_per_step": e2e_mean * 1e3,
                  "api": "kara_compress_window_host (pinned host window_q/tables in, tables + free count out)"}
                 if res["e2e"] else None),
+        # the same metric for the chain a serving engine runs on the device at a compression event: hidden states (resident)
+        # -> kara_window_queries_static (Q projection + RoPE) -> kara_compress_window, layer by layer; rank 0's mean
+        "e2e_device_chain": ({"value": res["wc_step"] / (res["chain"]["ms"] * 1e-3), "unit": UNIT,
+                              "ms_per_step": res["chain"]["ms"], "producer_ms": res["chain"]["producer_ms"],
+                              "compress_ms": res["chain"]["ms"] - res["chain"]["producer_ms"],
+                              "producer_tflops": res["chain"]["producer_flops"] / (res["chain"]["producer_ms"] * 1e-3) / 1e12,
+                              "steps": res["chain"]["steps"], "d_model": res["chain"]["d_model"],
+                              "window_tokens_per_layer": res["chain"]["tokens"],
+                              "hidden_bytes_resident": res["chain"]["hidden_bytes"], "h2d_bytes_per_step": 0,
+                              "gpu_launches_per_step": res["chain"]["launches"],
+                              "api": "per layer: kara_window_queries_static(hidden, W_q[l]) -> window_q[l]; "
+                                     "kara_compress_window(l, l+1), KARA_COMMIT on the last; synthetic hidden states"}
+                             if res["chain"] else None),
         "gpu_launches": res["launches"],
         # the same step with the library's two event records around the score launch switched off (they sit between the
         # score kernel and the select kernel that is launched programmatically behind it); rank 0's mean, same protocol
