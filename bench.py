@@ -92,18 +92,20 @@ def algorithmic(shape, L, qbuf_only=False):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE score-kernel launch, from the committed `ncu --set full`
-# captures of exactly these commands (profiles/r2_ncu_score.md), keyed by (workload, resident layers, variant).
+# captures of exactly these commands, keyed by (workload, resident layers, variant): cfg4 from the round-3 capture
+# (profiles/r3_ncu.md, commit 0e978c3), the others from round 2's (profiles/r2_ncu_score.md, commit 26d0175 — the score
+# kernel's SASS has not changed since).
 NCU_SCORE_TRAFFIC_BYTES = {("cfg2", 40, "full"): 257.957e6 + 4.504e6, ("cfg3", 8, "full"): 3212.377e6 + 20.670e6,
-                           ("cfg4", 2, "full"): 6435.954e6 + 30.069e6, ("cfg5", 8, "full"): 4827.730e6 + 32.882e6,
+                           ("cfg4", 2, "full"): 6434.983e6 + 30.275e6, ("cfg5", 8, "full"): 4827.730e6 + 32.882e6,
                            ("cfg4", 2, "qbuf_only"): 1229.311e6 + 19.162e6}
-NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_score.md (ncu --set full, dram rd+wr of one score-kernel launch of this workload)"
-# The captures were taken at this commit; the number is only reported while the score kernel's sources are still the
-# ones of that commit (sha256 over the files below, in this order) — otherwise `traffic` is null and `traffic_stale` true.
-NCU_TRAFFIC_COMMIT = "26d0175"
+NCU_TRAFFIC_SOURCE = ("profiles/r3_ncu.md for cfg4, profiles/r2_ncu_score.md for the other workloads "
+                      "(ncu --set full, dram rd+wr of one score-kernel launch of this workload)")
+# The number is only reported while the score kernel's sources are still the ones the captures describe (sha256 over the
+# files below, in this order) — otherwise `traffic` is null and `traffic_stale` true.
+NCU_TRAFFIC_COMMIT = "0e978c3 (cfg4) / 26d0175 (others)"
 SCORE_KERNEL_SOURCES = ("score_tc.cu", "score_tc_ptx.cuh", "score_tc.h")
-# (sources as of the round-3 clean-up: the trace / diagnostic switches and unused PTX helpers were removed after the capture;
-# `cuobjdump -sass` of score_tc.o is identical instruction for instruction before and after, so the capture still describes
-# this kernel)
+# (the sources of commit 0e978c3, the round-3 capture's; the round-2 captures predate the removal of the trace / diagnostic
+# switches and of unused PTX helpers, which left `cuobjdump -sass` of score_tc.o identical instruction for instruction)
 SCORE_KERNEL_SHA256_AT_CAPTURE = "766c3e9f98689d782663db473fe64f64d42b572f55dc1a68844662c106551abe"
 
 
