@@ -26,7 +26,9 @@
  *
  * Conventions.  Pointers marked [dev] are device memory OWNED BY THE CALLER (e.g. torch
  * tensors); [host] are host memory.  The library allocates nothing on the device except through
- * kara_compress_window_host's internal staging buffers.  Calls are asynchronous on `stream`
+ * kara_compress_window_host's internal staging buffers; its device image carries two static arrays on every GPU
+ * that loads it (1 MiB of rotary tables for kara_window_queries_static, 128 KiB of per-handle status words).
+ * Calls are asynchronous on `stream`
  * (a cudaStream_t passed as void*; NULL = legacy default stream) unless marked synchronous.
  * Every call returns 0 (KARA_OK) or a negative KARA_E* code and never throws or aborts;
  * kara_last_error() gives a thread-local message for the last failure.  Data-dependent faults
